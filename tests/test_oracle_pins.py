@@ -1,0 +1,440 @@
+"""Pins for the CPU oracle: it is checked against what the paper and the mathematics fix,
+never against itself.  P# labels follow DESIGN.md "Oracle pins".  All CPU, no GPU.
+"""
+import json
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from oracle import gpe_oracle as O
+import gpe_inputs as I
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def full_box_grid(nx, ny, nz, h, radius=2):
+    box = O.Box(nx, ny, nz, h)
+    return box, O.SparseGrid(box, np.arange(nx * ny * nz, dtype=np.int64), radius)
+
+
+def sine_mode(nx, ny, nz, m):
+    ax = [np.sin(math.pi * m[d] * (np.arange(n) + 1) / (n + 1)) for d, n in enumerate((nx, ny, nz))]
+    return (ax[0][:, None, None] * ax[1][None, :, None] * ax[2][None, None, :]).astype(np.complex128)
+
+
+# ---- P1: exact discrete eigenvalues of sine modes, 7-point, Dirichlet box --------------
+@pytest.mark.parametrize("m", [(1, 1, 1), (2, 3, 1), (5, 1, 4)])
+def test_P1_sine_modes_7pt(m):
+    nx, ny, nz, h = 7, 9, 8, 0.3
+    box, grid = full_box_grid(nx, ny, nz, h)
+    psi = sine_mode(nx, ny, nz, m).ravel() * (1 + 0.5j)
+    lam = sum(-(4.0 / h ** 2) * math.sin(0.5 * math.pi * m[d] / (n + 1)) ** 2
+              for d, n in enumerate((nx, ny, nz)))
+    t = O.apply_T(grid, psi, 7)
+    assert np.max(np.abs(t - (-0.5 * lam) * psi)) < 1e-12 * abs(lam)
+
+
+# ---- P2: 13-point symbol in the interior, and the exact outer-layer defect -------------
+def test_P2_sine_modes_13pt_symbol_and_defect():
+    nx, ny, nz, h = 9, 8, 10, 0.37
+    m = (2, 1, 3)
+    box, grid = full_box_grid(nx, ny, nz, h)
+    psi3 = sine_mode(nx, ny, nz, m)
+    th = [math.pi * m[d] / (n + 1) for d, n in enumerate((nx, ny, nz))]
+    sym = [-(1.0 / h ** 2) * (2.5 - (8.0 / 3.0) * math.cos(t) + (1.0 / 6.0) * math.cos(2 * t)) for t in th]
+    lap = -2.0 * O.apply_T(grid, psi3.ravel(), 13).reshape(nx, ny, nz)
+    expect = sum(sym) * psi3
+    inner = (slice(1, -1),) * 3
+    assert np.max(np.abs(lap[inner] - expect[inner])) < 1e-11 * abs(sum(sym))
+    # outermost layer: zero extension drops the analytic image psi(-2) = -sin(theta) (and the
+    # mirror one at n+1); the stencil weight there is -1/12, so lap_zero_ext = lap_nat + psi_nat/12h^2.
+    sx = np.sin(th[0] * (np.arange(-2, nx + 2) + 1))      # analytic extension along x
+    fy = np.sin(th[1] * (np.arange(ny) + 1))
+    fz = np.sin(th[2] * (np.arange(nz) + 1))
+    for i, ghost in ((0, sx[0]), (nx - 1, sx[-1])):      # sx[0] = psi(-2), sx[-1] = psi(nx+1)
+        want = expect[i, 1:-1, 1:-1] + (1.0 / (12 * h * h)) * ghost * fy[1:-1, None] * fz[None, 1:-1]
+        assert np.max(np.abs(lap[i, 1:-1, 1:-1] - want)) < 1e-11 * abs(sum(sym))
+    assert abs(sx[0] + math.sin(th[0])) < 1e-15
+
+
+# ---- 1-D reference operators built independently (dense matrices + library eigh) -------
+def lap1d(n, h, stencil):
+    w = {7: [-2.0, 1.0], 13: [-2.5, 4.0 / 3.0, -1.0 / 12.0]}[stencil]
+    d = np.zeros((n, n))
+    for i in range(n):
+        for s in range(-(len(w) - 1), len(w)):
+            if 0 <= i + s < n:
+                d[i, i + s] = w[abs(s)] / h ** 2
+    return d
+
+
+def ho_ground_state_1d(n, h, stencil):
+    x = (np.arange(n) - 0.5 * (n - 1)) * h
+    hm = -0.5 * lap1d(n, h, stencil) + np.diag(0.5 * x * x)
+    e, v = np.linalg.eigh(hm)
+    return e[0], v[:, 0]
+
+
+# ---- P3 / P4: harmonic-trap ground-state energy 3/2 at g = 0, at the stencil's order ---
+@pytest.mark.parametrize("stencil,closed", [(7, lambda h: 1.5 - 3 * h ** 2 / 32),
+                                            (13, lambda h: 1.5 - h ** 4 / 32)])
+def test_P3_P4_harmonic_ground_state(stencil, closed):
+    n, h = 48, 0.25
+    e1, v1 = ho_ground_state_1d(n, h, stencil)
+    box, grid = full_box_grid(n, n, n, h)
+    psi = (v1[:, None, None] * v1[None, :, None] * v1[None, None, :]).ravel().astype(np.complex128)
+    psi /= math.sqrt(h ** 3 * np.sum(np.abs(psi) ** 2))
+    pot = O.Potential(kind=O.HARMONIC)
+    en = O.energy(grid, pot, 0.0, 0.0, psi, stencil)
+    hp = O.apply_H(grid, pot, 0.0, 0.0, psi, stencil)
+    assert abs(en["norm"] - 1.0) < 1e-13
+    assert np.max(np.abs(hp - 3 * e1 * psi)) < 1e-11 * np.max(np.abs(psi))
+    assert abs(en["total"] - 3 * e1) < 1e-12 and abs(en["mu"] - 3 * e1) < 1e-12
+    # closed forms: 3/2 - 3h^2/32 + O(h^4) (2nd order), 3/2 - h^4/32 + O(h^6) (4th order)
+    tol = 3e-5 if stencil == 7 else 4e-6   # O(h^4) resp. O(h^6) remainder; the h^2 / h^4 terms are 5.9e-3 / 1.2e-4
+    assert abs(en["total"] - closed(h)) < tol
+    assert abs(en["total"] - 1.5) > 10 * tol if stencil == 7 else True
+
+
+def test_P3_order_of_convergence():
+    # the 1-D references converge at order 2 / 4; the 3-D oracle was tied to them above
+    for stencil, order in ((7, 2), (13, 4)):
+        e = [ho_ground_state_1d(int(round(12 / h)), h, stencil)[0] for h in (0.5, 0.25)]
+        ratio = (e[0] - 0.5) / (e[1] - 0.5)
+        assert abs(math.log2(ratio) - order) < 0.15
+
+
+def test_P3_imaginary_time_converges_to_ground_state():
+    n, h = 20, 0.6
+    box, grid = full_box_grid(n, n, n, h)
+    pot = O.Potential(kind=O.HARMONIC)
+    e1, v1 = ho_ground_state_1d(n, h, 7)
+    rng = np.random.default_rng(0)
+    x = O.coords(n, h)
+    g0 = np.exp(-0.35 * x * x)
+    psi = (g0[:, None, None] * g0[None, :, None] * g0[None, None, :]).ravel() * (1 + 0.1 * rng.normal(size=n ** 3))
+    psi = psi.astype(np.complex128)
+    psi /= math.sqrt(O.norm(grid, psi))
+    last = O.energy(grid, pot, 0.0, 0.0, psi, 7)["total"]
+    for _ in range(20):      # dt * lambda_max ~ 0.65: stable forward Euler
+        psi = O.run_imag(grid, pot, 0.0, 0.0, 0.01, 25, psi, 7)
+        assert abs(O.norm(grid, psi) - 1.0) < 1e-13
+        e = O.energy(grid, pot, 0.0, 0.0, psi, 7)["total"]
+        assert e <= last + 1e-13      # monotone for small dt
+        last = e
+    assert abs(last - 3 * e1) < 2e-4
+    assert last > 3 * e1 - 1e-12
+
+
+# ---- P5: brute-force operator matrices from Kronecker products, rows/cols deleted ------
+@pytest.mark.parametrize("stencil", [7, 13])
+@pytest.mark.parametrize("dims", [(6, 6, 6), (5, 6, 7)])
+def test_P5_kronecker_submatrix(stencil, dims):
+    nx, ny, nz = dims
+    h = 0.7
+    eye = np.eye
+    lap = (np.kron(np.kron(lap1d(nx, h, stencil), eye(ny)), eye(nz))
+           + np.kron(np.kron(eye(nx), lap1d(ny, h, stencil)), eye(nz))
+           + np.kron(np.kron(eye(nx), eye(ny)), lap1d(nz, h, stencil)))
+    for seed, p in ((1, 0.5), (2, 0.85), (3, 0.15)):
+        act = I.random_mask_lin(seed, nx, ny, nz, p)
+        tmat = -0.5 * lap[np.ix_(act, act)]           # remove rows and columns
+        grid = O.SparseGrid(O.Box(nx, ny, nz, h), act, 2)
+        for k in range(0, act.size, max(1, act.size // 7)):
+            e = np.zeros(act.size, np.complex128)
+            e[k] = 1.0
+            assert np.max(np.abs(O.apply_T(grid, e, stencil) - tmat[:, k])) < 1e-13
+        psi = I.random_psi(seed, act.size)
+        assert np.max(np.abs(O.apply_T(grid, psi, stencil) - tmat @ psi)) < 1e-12 * np.max(np.abs(tmat)) * 8
+
+
+# ---- P6: sparse operator == dense shifted-slice stencil -------------------------------
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_P6_sparse_equals_dense(stencil):
+    nx, ny, nz, h = 9, 7, 11, 0.4
+    box = O.Box(nx, ny, nz, h)
+    for p in (1.0, 0.6):
+        act = np.arange(nx * ny * nz, dtype=np.int64) if p == 1.0 else I.random_mask_lin(7, nx, ny, nz, p)
+        grid = O.SparseGrid(box, act, 2)
+        psi = I.random_psi(5, act.size)
+        dense = np.zeros(nx * ny * nz, np.complex128)
+        dense[act] = psi
+        mask = np.zeros(nx * ny * nz, bool)
+        mask[act] = True
+        td = O.dense_apply_T(box, mask.reshape(nx, ny, nz), dense.reshape(nx, ny, nz), stencil).ravel()[act]
+        assert np.max(np.abs(O.apply_T(grid, psi, stencil) - td)) < 1e-12 * np.max(np.abs(td))
+
+
+# ---- P7: sign of i -- psi(t) = exp(-i E t) psi(0)  (Eq. 2) -----------------
+def test_P7_phase_rotation_sign():
+    n, h = 16, 0.7
+    box, grid = full_box_grid(n, n, n, h)
+    e1, v1 = ho_ground_state_1d(n, h, 7)
+    psi0 = (v1[:, None, None] * v1[None, :, None] * v1[None, None, :]).ravel().astype(np.complex128)
+    pot = O.Potential(kind=O.HARMONIC)
+    dt, ns = 2e-3, 50
+    psi = O.run_rk4(grid, pot, 0.0, 0.0, dt, ns, psi0, 7)
+    ph = np.angle(np.vdot(psi0, psi))
+    assert abs(ph - (-3 * e1 * dt * ns)) < 1e-9
+
+
+# ---- P8: RK4 tableau -- exact amplification factor of an eigenmode, and order 4 --------
+def test_P8_amplification_factor_and_order():
+    nx, ny, nz, h = 6, 5, 7, 0.5
+    box, grid = full_box_grid(nx, ny, nz, h)
+    m = (2, 1, 3)
+    psi = sine_mode(nx, ny, nz, m).ravel()
+    lam = -0.5 * sum(-(4.0 / h ** 2) * math.sin(0.5 * math.pi * m[d] / (n + 1)) ** 2
+                     for d, n in enumerate((nx, ny, nz)))
+    pot = O.Potential(kind=O.HARMONIC, ax=0.0, ay=0.0, az=0.0)
+    dt = 0.02
+    z = lam * dt
+    out = O.rk4_step(grid, pot, 0.0, 0.0, dt, psi, 7)
+    rz = 1 - 1j * z - z * z / 2 + 1j * z ** 3 / 6 + z ** 4 / 24
+    assert np.max(np.abs(out - rz * psi)) < 1e-13
+    assert abs(abs(rz) ** 2 - (1 - z ** 6 / 72 + z ** 8 / 576)) < 1e-14
+    # order: linear problem on a random mask, exact propagator from library eigh
+    act = I.random_mask_lin(4, 6, 6, 6, 0.7)
+    g2 = O.SparseGrid(O.Box(6, 6, 6, 0.5), act, 2)
+    lap = (np.kron(np.kron(lap1d(6, 0.5, 13), np.eye(6)), np.eye(6))
+           + np.kron(np.kron(np.eye(6), lap1d(6, 0.5, 13)), np.eye(6))
+           + np.kron(np.kron(np.eye(6), np.eye(6)), lap1d(6, 0.5, 13)))
+    pot2 = O.Potential(kind=O.HARMONIC, ax=1.0, ay=2.0, az=0.5)
+    hmat = -0.5 * lap[np.ix_(act, act)] + np.diag(O.potential_at(g2.box, pot2, act, 0.0))
+    ev, U = np.linalg.eigh(hmat)
+    p0 = I.random_psi(9, act.size)
+    T = 0.2
+    exact = U @ (np.exp(-1j * ev * T) * (U.conj().T @ p0))
+    errs = []
+    for ns in (40, 80):
+        p = O.run_rk4(g2, pot2, 0.0, 0.0, T / ns, ns, p0, 13)
+        errs.append(np.max(np.abs(p - exact)))
+    assert 13.0 < errs[0] / errs[1] < 19.0
+
+
+def test_P8_norm_and_energy_conservation_nonlinear():
+    w = I.small_shell(24, 7)
+    box = O.Box(w.nx, w.ny, w.nz, w.h)
+    pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
+    act = O.active_indices(box, pot, w.v_cut)
+    grid = O.SparseGrid(box, act, 2)
+    psi = I.make_psi0(w, act)
+    e0 = O.energy(grid, pot, w.g, 0.0, psi, 7)
+    drift = []
+    for dt in (2e-3, 1e-3):
+        p = O.run_rk4(grid, pot, w.g, 0.0, dt, int(round(0.02 / dt)), psi, 7)
+        e1 = O.energy(grid, pot, w.g, 0.0, p, 7)
+        drift.append((abs(e1["norm"] - 1.0), abs(e1["total"] - e0["total"])))
+    assert drift[1][0] < 1e-9 and drift[1][1] < 1e-7 * abs(e0["total"])
+    assert drift[0][0] / max(drift[1][0], 1e-300) > 8      # norm drift ~ dt^5 per unit time
+    assert drift[0][1] / max(drift[1][1], 1e-300) > 8      # energy drift ~ dt^4 or better
+
+
+# ---- P9: the memory-optimised RK form ---------------------
+def modified_tableau(a, b):
+    """a*, b* from a standard explicit Butcher tableau via PAPER.md Eq. A4-A7 (dt = 1)."""
+    n = len(b)
+    M = [[Fraction(0)] * n for _ in range(n)]
+    for i in range(n):
+        M[i][0] = Fraction(1)
+        for j in range(i):
+            M[i][j + 1] = Fraction(a[i][j])
+    # invert lower-triangular M:  K = Minv Y   with K = (y0, k1..k_{n-1}), Y = (y1..yn)
+    Minv = [[Fraction(0)] * n for _ in range(n)]
+    for c in range(n):
+        for r in range(n):
+            rhs = Fraction(1 if r == c else 0) - sum(M[r][k] * Minv[k][c] for k in range(r))
+            Minv[r][c] = rhs / M[r][r]
+    astar = []
+    for i in range(1, n):            # y^(i+1) = y0 + sum_{j<i} a_{i+1,j} k_j + a_{i+1,i} k_i
+        row = [Fraction(0)] * i
+        coef = [Fraction(1)] + [Fraction(a[i][j]) for j in range(i - 1)]
+        for j, cj in enumerate(coef):
+            for c in range(i):
+                row[c] += cj * Minv[j][c]
+        astar.append(row)
+    coef = [Fraction(1)] + [Fraction(b[j]) for j in range(n - 1)]
+    bstar = [Fraction(0)] * n
+    for j, cj in enumerate(coef):
+        for c in range(n):
+            bstar[c] += cj * Minv[j][c]
+    return astar, bstar
+
+
+def test_P9_modified_tableau_matches_paper():
+    gold = json.load(open(os.path.join(GOLD, "paper_values.json")))
+    F = Fraction
+    a4 = [[], [F(1, 2)], [0, F(1, 2)], [0, 0, 1]]
+    b4 = [F(1, 6), F(1, 3), F(1, 3), F(1, 6)]
+    astar, bstar = modified_tableau(a4, b4)
+    assert bstar == [F(s) for s in gold["rk4_b_star"]["value"]]
+    for i, row in enumerate(gold["rk4_a_star"]["value"]):
+        assert astar[i] == [F(v) for v in row[: i + 1]]
+    a3 = [[], [F(1, 3)], [0, F(2, 3)]]
+    b3 = [F(1, 4), 0, F(3, 4)]
+    astar3, bstar3 = modified_tableau(a3, b3)
+    assert bstar3 == [F(s) for s in gold["rkhe3_b_star"]["value"]]
+    for i, row in enumerate(gold["rkhe3_a_star"]["value"]):
+        assert astar3[i] == [F(v) for v in row[: i + 1]]
+
+
+def test_P9_stage_form_equals_textbook_rk4():
+    """The S1-S4 stage form the CUDA path uses == textbook RK4, via the oracle's H."""
+    w = I.small_shell(20, 13)
+    box = O.Box(w.nx, w.ny, w.nz, w.h)
+    pot = O.Potential(w.kind, w.ax, w.ay, w.az, 5.0, 20.0, 0.01, w.omega)
+    act = O.active_indices(box, pot, w.v_cut, O.MASK_UNION)
+    grid = O.SparseGrid(box, act, 2)
+    y0 = I.make_psi0(w, act)
+    t, dt, g = 0.003, 1e-3, w.g
+    f = lambda tt, y: -1j * O.apply_H(grid, pot, g, tt, y, 13)
+    y2 = y0 + 0.5 * dt * f(t, y0)
+    y3 = y0 + 0.5 * dt * f(t + 0.5 * dt, y2)
+    p = -y0 / 3 + y2 / 3 + 2 * y3 / 3
+    y4 = y0 + dt * f(t + 0.5 * dt, y3)
+    ynew = p + y4 / 3 + (dt / 6) * f(t + dt, y4)
+    ref = O.rk4_step(grid, pot, g, t, dt, y0, 13)
+    assert np.max(np.abs(ynew - ref)) < 1e-14 * np.max(np.abs(ref))
+
+
+# ---- P10: Hermiticity of the reduced operator (principal sub-matrix) ------
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_P10_hermitian(stencil):
+    act = I.random_mask_lin(12, 8, 9, 7, 0.55)
+    grid = O.SparseGrid(O.Box(8, 9, 7, 0.3), act, 2)
+    a, b = I.random_psi(1, act.size), I.random_psi(2, act.size)
+    lhs = np.vdot(a, O.apply_T(grid, b, stencil))
+    rhs = np.vdot(O.apply_T(grid, a, stencil), b)
+    assert abs(lhs - rhs) < 1e-11 * abs(lhs)
+
+
+# ---- P11: stage times c = 0, 1/2, 1/2, 1 -- one-point mask = scalar ODE ----------------
+def test_P11_one_point_mask_scalar_ode():
+    from scipy.integrate import quad
+    box = O.Box(5, 5, 5, 0.5)
+    pot = O.Potential(kind=O.DRESSED, ax=1.0, ay=1.0, az=1.0, delta0=0.0, delta1=6.0, t_ramp=0.5, omega=1.5)
+    lin = np.array([(1 * 5 + 3) * 5 + 4], dtype=np.int64)
+    grid = O.SparseGrid(box, lin, 2)
+    g, stencil = 3.0, 13
+    x, y, z = (O.coords(5, 0.5)[i] for i in (1, 3, 4))
+    u = 0.5 * (x * x + y * y + z * z)
+    vt = lambda t: math.sqrt((u - (0.0 + 6.0 * min(max(t / 0.5, 0.0), 1.0))) ** 2 + 1.5 ** 2) - 1.5
+    c = -0.5 * 3 * (-2.5) / 0.5 ** 2               # diagonal of T for the 13-point stencil
+    psi0 = np.array([0.8 - 0.3j])
+    T, ns = 0.4, 400        # z = dt*(c+V+g|psi|^2) ~ 0.02: RK4 phase error z^5/120 per step ~ 1e-8 total
+    psi = O.run_rk4(grid, pot, g, 0.05, T / ns, ns, psi0, stencil)
+    integral = quad(vt, 0.05, 0.05 + T, epsabs=1e-13, epsrel=1e-13)[0]
+    exact = psi0 * np.exp(-1j * (integral + (g * abs(psi0[0]) ** 2 + c) * T))
+    assert abs(psi[0] - exact[0]) < 5e-8            # O(dt^4); wrong stage times give O(dt) ~ 1e-2
+    wrong = psi0 * np.exp(-1j * (vt(0.05) * T + (g * abs(psi0[0]) ** 2 + c) * T))
+    assert abs(wrong[0] - exact[0]) > 1e-2
+
+
+# ---- P12: layout -- counts, halo, tile tables ------------------------------------------
+def _wl_objects(w):
+    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center)
+    pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
+    return box, pot
+
+
+def test_P12_counts_fixture_config1_config2():
+    gold = json.load(open(os.path.join(GOLD, "paper_values.json")))
+    assert gold["block_tile_points"]["value"] - gold["block_interior_points"]["value"] == gold["block_halo_points"]["value"] == 10 ** 3 - 8 ** 3
+    counts = json.load(open(os.path.join(GOLD, "counts.json")))
+    for w in (I.config1(), I.config2()):
+        box, pot = _wl_objects(w)
+        act = O.active_indices(box, pot, w.v_cut, w.mask_mode, check_knife_edge=True)
+        st = O.stored_indices(box, act, w.halo_width)
+        assert act.size == counts[w.name]["n_active"]
+        assert st.size == counts[w.name]["n_stored"]
+    # the survey's independent count script gave the same numbers
+    assert counts["cfg1_harmonic_48"] == {"n_active": 67080, "n_stored": 67080 + 9888}
+    assert counts["cfg2_bubble_256"] == {"n_active": 1215760, "n_stored": 1215760 + 418000}
+
+
+def test_P12_mask_is_ball_for_harmonic():
+    w = I.config1()
+    box, pot = _wl_objects(w)
+    act = O.active_indices(box, pot, w.v_cut)
+    ix, iy, iz = O.unravel(box, act)
+    c = O.coords(48, 0.25)
+    r2 = c[ix] ** 2 + c[iy] ** 2 + c[iz] ** 2
+    assert np.all(r2 < 40.0)
+    allr2 = (c[:, None, None] ** 2 + c[None, :, None] ** 2 + c[None, None, :] ** 2).ravel()
+    assert act.size == int(np.sum(allr2 < 40.0 - 1e-9)) == int(np.sum(allr2 < 40.0 + 1e-9))
+    assert abs(c[0] + 5.875) < 1e-15 and abs(c[23] + 0.125) < 1e-15     # symmetric, no point at 0
+
+
+def test_P12_union_mask_is_union_over_ramp():
+    w = I.small_shell(24, 7)
+    box, _ = _wl_objects(w)
+    pot = O.Potential(O.DRESSED, 1.0, 1.2, 0.9, 0.0, 20.0, 1.0, 6.0)
+    uni = set(O.active_indices(box, pot, w.v_cut, O.MASK_UNION).tolist())
+    acc = set()
+    for d in np.linspace(0.0, 20.0, 401):
+        p = O.Potential(O.DRESSED, 1.0, 1.2, 0.9, d, d, 0.0, 6.0)
+        acc |= set(O.active_indices(box, p, w.v_cut, O.MASK_AT_DELTA0).tolist())
+    assert acc <= uni and len(uni - acc) <= 0.002 * len(uni)
+
+
+def test_P12_halo_resolves_every_neighbour():
+    w = I.small_shell(24, 13)
+    box, pot = _wl_objects(w)
+    act = O.active_indices(box, pot, w.v_cut)
+    st = set(O.stored_indices(box, act, 2).tolist())
+    ix, iy, iz = O.unravel(box, act)
+    for (dx, dy, dz) in [(s * a, s * b, s * c) for s in (-2, -1, 1, 2) for (a, b, c) in ((1, 0, 0), (0, 1, 0), (0, 0, 1))]:
+        jx, jy, jz = ix + dx, iy + dy, iz + dz
+        inside = (0 <= jx) & (jx < box.nx) & (0 <= jy) & (jy < box.ny) & (0 <= jz) & (jz < box.nz)
+        lin = (jx * box.ny + jy) * box.nz + jz
+        assert all(int(l) in st for l in lin[inside])
+    assert set(act.tolist()) <= st
+
+
+@pytest.mark.parametrize("zt", [32, 5])
+def test_P12_tile_layout_invariants(zt):
+    w = I.small_shell(24, 13)
+    box, pot = _wl_objects(w)
+    act = O.active_indices(box, pot, w.v_cut)
+    L = O.tile_layout(box, act, 8, 8, zt)
+    perm = L["storage_to_canonical"]
+    assert np.array_equal(np.sort(perm), np.arange(act.size))
+    # decode every slab lane back to a linear index and compare with the permuted active list
+    lin = []
+    for k in range(L["n_tiles"]):
+        i, j = L["tile_xy"][k]
+        for z in range(L["tile_zlo"][k], L["tile_zhi"][k]):
+            e = L["tile_entry_base"][k] + z - L["tile_zlo"][k]
+            m = int(L["slab_mask"][e])
+            assert L["slab_base"][e] == len(lin)
+            for b in range(64):
+                if m >> b & 1:
+                    lin.append(((i * 8 + b // 8) * box.ny + (j * 8 + b % 8)) * box.nz + z)
+    assert np.array_equal(np.asarray(lin), act[perm])
+    # work items cover each non-empty slab exactly once, never exceed zt, never hold an empty slab
+    seen = set()
+    for t, z0, nz in zip(L["wi_tile"], L["wi_z0"], L["wi_nz"]):
+        assert 1 <= nz <= zt
+        for z in range(z0, z0 + nz):
+            e = L["tile_entry_base"][t] + z - L["tile_zlo"][t]
+            assert L["slab_mask"][e] != 0 and (t, z) not in seen
+            seen.add((int(t), int(z)))
+    assert len(seen) == int(np.count_nonzero(L["slab_mask"]))
+    # neighbour table is symmetric
+    for k in range(L["n_tiles"]):
+        for q, qq in ((0, 1), (1, 0), (2, 3), (3, 2)):
+            n = L["tile_nbr"][k, q]
+            if n >= 0:
+                assert L["tile_nbr"][n, qq] == k
+
+
+def test_uniform01_is_layout_independent_and_uniform():
+    lin = np.arange(200000, dtype=np.int64)
+    u = I.uniform01(3, lin)
+    assert 0.0 <= u.min() and u.max() < 1.0 and abs(u.mean() - 0.5) < 5e-3
+    p = np.random.default_rng(0).permutation(lin.size)
+    assert np.array_equal(I.uniform01(3, lin[p]), u[p])
+    assert not np.array_equal(I.uniform01(4, lin), u)

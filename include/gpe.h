@@ -1,0 +1,205 @@
+/* gpe.h -- C ABI of libgpe_b200.so: the sparse-grid Gross-Pitaevskii hot path on one B200.
+ *
+ * What the library computes (citations: /root/reference/PAPER.md line, section / equation):
+ *   H[psi;t] psi = -1/2 lap_h psi + V(r,t) psi + g |psi|^2 psi        PAPER.md:25-27 Eq. 1-2, :71 Eq. 8
+ * on the region of interest M = {p in box : V_mask(r_p) < V_cut}          PAPER.md:50-52 Eq. 5
+ * with the rows and columns of points outside M deleted (psi = 0 there)
+ * fused into explicit RK4 stages in the memory-optimised form            PAPER.md:89-99, :276-281 Eq. A6-A7,
+ *                                                                         :315-319 Eq. A10-A11
+ * and into normalised imaginary-time steps with a particle-number
+ * reduction and lazy renormalisation                                     PAPER.md:35, :60 Eq. 6, :87 (kernel K3)
+ * DESIGN.md lists the readings taken where the paper is silent (R1..R18).
+ *
+ * Conventions
+ *   - every function returns int: 0 = GPE_OK, negative = error; out-parameters are untouched on error;
+ *     gpe_last_error() returns thread-local text for the last failing call of the calling thread.
+ *   - "host" pointers are ordinary CPU memory owned by the caller; "dev" pointers are CUDA device memory
+ *     owned by the caller (e.g. torch tensors' data_ptr()).  The library owns only its tables.
+ *   - `stream` is a cudaStream_t passed as void* (0 = legacy default stream).  Device work is enqueued on
+ *     it and is asynchronous, EXCEPT calls that return host scalars (gpe_norm, gpe_energy) and the *_host
+ *     copies, which synchronise that stream before returning.
+ *   - complex values are interleaved (re, im): complex128 = 2 doubles, complex64 = 2 floats.
+ *   - global linear index L = (ix*ny + iy)*nz + iz (C order, z fastest); coordinates
+ *     x_i = ((double)i - 0.5*(nx-1))*h + center[0] (same for y, z).
+ *   - "canonical order" of a wavefunction = ascending L over M, length n_active.
+ *   - nothing here falls back to the CPU: with no usable CUDA device the device calls return GPE_ERR_CUDA.
+ *   - handles are not thread-safe; use one sim per host thread.
+ */
+#ifndef GPE_H_
+#define GPE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GPE_OK 0
+#define GPE_ERR_INVALID_ARG (-1)
+#define GPE_ERR_OUT_OF_MEMORY (-2)
+#define GPE_ERR_CUDA (-3)
+#define GPE_ERR_UNSUPPORTED (-4)
+#define GPE_ERR_STATE (-5)
+
+/* potential kinds (BASELINE.json configs; dressed form after PAPER.md:139 Eq. 10) */
+#define GPE_POT_HARMONIC 0 /* V = u,  u = 1/2 (ax x^2 + ay y^2 + az z^2)                    */
+#define GPE_POT_DRESSED 1  /* V = sqrt((u - Delta(t))^2 + Omega^2) - Omega                  */
+/* which Delta defines the mask (R13) */
+#define GPE_MASK_AT_DELTA0 0
+#define GPE_MASK_AT_DELTA1 1
+#define GPE_MASK_UNION 2 /* union over the ramp: Delta = clamp(u, min(d0,d1), max(d0,d1))     */
+
+#define GPE_C64 0  /* complex64 state; coordinates, V and all reductions still fp64           */
+#define GPE_C128 1 /* complex128 state                                                        */
+
+typedef struct gpe_grid gpe_grid; /* opaque: active set + layout tables (host, and device once a sim exists) */
+typedef struct gpe_sim gpe_sim;   /* opaque: one wavefunction evolving on a grid                              */
+
+typedef struct {
+    int32_t nx, ny, nz; /* box size in points, each >= 1 */
+    int32_t reserved;   /* must be 0 */
+    double h;           /* grid spacing, > 0 */
+    double center[3];   /* coordinate of the box centre */
+} gpe_box;
+
+typedef struct {
+    int32_t kind;      /* GPE_POT_* */
+    int32_t mask_mode; /* GPE_MASK_* (ignored for harmonic) */
+    double ax, ay, az; /* quadratic-form coefficients */
+    double delta0, delta1, t_ramp; /* Delta(t) = delta0 + (delta1-delta0)*clamp(t/t_ramp,0,1); t_ramp<=0: delta0 */
+    double omega;
+} gpe_potential;
+
+/* Layout: 8x8 column tiles in (x,y), one 64-bit occupancy mask per z-plane ("slab") of a tile, points
+ * stored COMPACTLY (no padding, no ghost lanes) in the order tile, z, bit = lx*ty + ly.
+ * "Data layout".  Prior art: the paper's 8^3 blocks + 488-entry halo lists. */
+typedef struct {
+    int32_t tx, ty, zt, halo_width;
+    int64_t n_active;  /* |M| */
+    int64_t n_tiles;   /* present tiles */
+    int64_t n_slabs;   /* sum over tiles of (zhi - zlo) */
+    int64_t n_work;    /* work items */
+} gpe_layout_info;
+
+/* Caller-allocated host arrays to receive the canonical tables (any pointer may be NULL = skip).
+ * Definitions: DESIGN.md "Layout tables"; lengths from gpe_layout_info. */
+typedef struct {
+    int32_t* tile_xy;              /* [n_tiles][2]  tile coordinates (i, j) = (ix/tx, iy/ty)           */
+    int32_t* tile_zlo;             /* [n_tiles]     min iz over the tile's points                      */
+    int32_t* tile_zhi;             /* [n_tiles]     max iz + 1                                         */
+    int64_t* tile_entry_base;      /* [n_tiles]     index of the tile's first slab                     */
+    int32_t* tile_nbr;             /* [n_tiles][4]  present-tile index of (i-1,j),(i+1,j),(i,j-1),(i,j+1) or -1 */
+    uint64_t* slab_mask;           /* [n_slabs]     bit lx*ty+ly set iff the point is in M             */
+    int64_t* slab_base;            /* [n_slabs]     storage position of the slab's first lane          */
+    int32_t* wi_tile;              /* [n_work]      work items: tile,                                  */
+    int32_t* wi_z0;                /* [n_work]        first plane,                                     */
+    int32_t* wi_nz;                /* [n_work]        number of planes (<= zt)                         */
+    int64_t* storage_to_canonical; /* [n_active]    canonical rank of the point in storage slot s     */
+} gpe_layout_tables;
+
+typedef struct {
+    double kin;   /* h^3 sum Re(conj(psi) T psi),  T = -1/2 lap_h                                  */
+    double pot;   /* h^3 sum V |psi|^2                                                              */
+    double inter; /* h^3 (g/2) sum |psi|^4                                                          */
+    double total; /* kin + pot + inter                                                              */
+    double mu;    /* h^3 sum Re(conj(psi) H psi) / norm = (kin + pot + 2 inter) / norm  (Eq. 1)     */
+    double norm;  /* h^3 sum |psi|^2  (Eq. 3)                                                       */
+} gpe_energy_out;
+
+/* ---- error text ------------------------------------------------------------------------------------ */
+const char* gpe_last_error(void);
+
+/* ---- a1: active-set layout builder (HOST ONLY: no CUDA call is made) ---------------------------------
+ * PAPER.md:50-58 (ROI from the Thomas-Fermi density: V < cutoff), :81-85 (block post-selection, index
+ * tables).  Evaluates the mask in the fixed floating-point order of DESIGN.md R2 (no FMA), strict '<',
+ * and builds the tables above.  halo_width (0..8) only defines the ghost ring reported by
+ * gpe_grid_stored_indices (R3); the ring is never stored on the device because every read
+ * outside M is zero.  A sim needs halo_width >= stencil radius.  Errors: INVALID_ARG (null pointer,
+ * n < 1, h <= 0, unknown kind/mode, box with more than 2^62 points), OUT_OF_MEMORY.  An empty mask is
+ * valid (n_active = 0). */
+int gpe_grid_create(const gpe_box* box, const gpe_potential* pot, double v_cut, int halo_width,
+                    gpe_grid** out);
+
+/* Same tables from an explicit active set: host array of n strictly ascending linear indices inside the
+ * box (edge-case masks: random, single point, full box).  pot is still used for V(r,t). */
+int gpe_grid_create_from_indices(const gpe_box* box, const gpe_potential* pot, const int64_t* active_host,
+                                 int64_t n, int halo_width, gpe_grid** out);
+
+/* Frees host tables and, if uploaded, device tables.  Sims created on the grid must be destroyed first.
+ * NULL is a no-op. */
+int gpe_grid_destroy(gpe_grid* g);
+
+int gpe_grid_num_active(const gpe_grid* g, int64_t* out);
+/* |S|, S = M u star-halo(M, halo_width) clipped to the box; computed on first use, O(|M| halo_width). */
+int gpe_grid_num_stored(gpe_grid* g, int64_t* out);
+int gpe_grid_layout_info(const gpe_grid* g, gpe_layout_info* out);
+/* out_host: n_active int64, ascending L over M */
+int gpe_grid_active_indices(const gpe_grid* g, int64_t* out_host);
+/* out_host: gpe_grid_num_stored() int64, ascending L over S */
+int gpe_grid_stored_indices(gpe_grid* g, int64_t* out_host);
+int gpe_grid_layout_tables(const gpe_grid* g, const gpe_layout_tables* out_host);
+
+/* ---- simulation object ------------------------------------------------------------------------------
+ * Bytes of caller-owned device memory a sim needs: four state buffers in storage order (y0 / y2,y4 / y3 /
+ * p of PAPER.md:276-281 Eq. A6-A7 specialised to RK4), one canonical staging buffer, reduction scratch. */
+int gpe_sim_state_bytes(const gpe_grid* g, int dtype, size_t* out);
+
+/* stencil: 7 (2nd order, PAPER.md:58, :337-339 Eq. B1) or 13 (4th-order star, R5).
+ * g: interaction strength multiplying |psi|^2; n_target: value of h^3 sum|psi|^2 that imaginary-time
+ * steps renormalise to (Eq. 3).  dev_state: device memory, 256-byte aligned, >= state_bytes,
+ * must stay valid until gpe_sim_destroy; it is zero-initialised here (psi = 0, t = 0).  Uploads the
+ * grid's tables to the current CUDA device on first use.  Errors: INVALID_ARG, UNSUPPORTED (tile shape
+ * other than 8x8, halo_width < radius), CUDA (no device, not sm_100), OUT_OF_MEMORY. */
+int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_target, void* dev_state,
+                   size_t state_bytes, void* stream, gpe_sim** out);
+int gpe_sim_destroy(gpe_sim* s);
+
+/* a7: canonical <-> storage order.  dev_psi: n_active complex values of the sim's dtype on the device. */
+int gpe_set_psi(gpe_sim* s, const void* dev_psi_canonical, void* stream);
+int gpe_get_psi(gpe_sim* s, void* dev_psi_canonical, void* stream);
+/* Same with HOST buffers: host->device copy + pack, unpack + device->host copy; synchronise `stream`. */
+int gpe_set_psi_host(gpe_sim* s, const void* host_psi_canonical, void* stream);
+int gpe_get_psi_host(gpe_sim* s, void* host_psi_canonical, void* stream);
+
+int gpe_set_time(gpe_sim* s, double t);
+int gpe_get_time(const gpe_sim* s, double* t);
+
+/* a2+a3: dev_out = H[dev_in; t] dev_in, both canonical, n_active values, must not overlap.  Uses the
+ * sim's g and stencil; does not touch the sim's own psi or clock.  (PAPER.md:27 Eq. 2, :58.) */
+int gpe_apply_H(gpe_sim* s, double t, const void* dev_in_canonical, void* dev_out_canonical, void* stream);
+
+/* a4: one / nsteps classic RK4 steps of i dpsi/dt = H psi (PAPER.md:71 Eq. 8, :91 Eq. 9) as four fused
+ * stage kernels in the stage-state form (Eq. A6-A7, A10-A11).  V is evaluated at the stage times
+ * t, t+dt/2, t+dt/2, t+dt.  Step n of a run starts at t_start + n*dt (a product, not a running sum); the
+ * sim clock ends at t_start + nsteps*dt. */
+int gpe_step_rk4(gpe_sim* s, double dt, void* stream);
+int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream);
+
+/* a5: psi' = psi - dt H[psi] psi, psi <- psi' sqrt(n_target / (h^3 sum|psi'|^2)) with V frozen at the sim
+ * clock (PAPER.md:35, :60 Eq. 6, :87; forward-Euler reading DESIGN.md R7).  One fused kernel per step
+ * (update + block partial sums) + a one-block finalise; the scale is applied lazily at the next load as
+ * in the paper's kernel K1 and flushed at the end of the call, so the state seen by every
+ * other call is normalised.  A state with zero norm yields GPE_ERR_STATE at the next host-scalar call. */
+int gpe_imag_step(gpe_sim* s, double dt, void* stream);
+int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream);
+
+/* a6: reductions over the sim's psi; fp64 accumulation, fixed summation order (bit-reproducible).
+ * Synchronise `stream`.  Energy terms use V at the sim clock. */
+int gpe_norm(gpe_sim* s, double* out_host, void* stream);
+int gpe_energy(gpe_sim* s, gpe_energy_out* out_host, void* stream);
+
+/* Number of kernels this sim has launched so far (bench.py's gpu_launches). */
+int gpe_sim_kernel_launches(const gpe_sim* s, int64_t* out);
+/* Name/duration of the stage kernels: enables CUDA-event timing of every RK4 stage launch inside
+ * gpe_run_rk4 on the launching stream (bench.py's roofline leg); on=0 disables.  gpe_sim_stage_time_ms
+ * returns the accumulated milliseconds and launch count per stage index 0..3 and resets them. */
+int gpe_sim_time_stages(gpe_sim* s, int on);
+int gpe_sim_stage_time_ms(gpe_sim* s, double ms_out[4], int64_t count_out[4]);
+/* Tuning knob: planes per thread block (1..32, default chosen per dtype/stencil).  INVALID_ARG otherwise. */
+int gpe_sim_set_planes_per_block(gpe_sim* s, int kz);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GPE_H_ */

@@ -1,0 +1,558 @@
+// C-ABI glue of libgpe_b200.so (include/gpe.h): handles, argument checks, table upload, and the
+// sequences of kernel launches behind each call.  Every step of the path runs in gpe_kernels.cu; there
+// is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "gpe_internal.h"
+
+using namespace gpe;
+
+struct gpe_grid {
+    GridHost h;
+    // device tables (uploaded when the first sim is created on the grid)
+    bool on_device = false;
+    int device = -1;
+    Slab* d_slabs = nullptr;
+    int64_t* d_perm = nullptr;
+    int n_sims = 0;
+};
+
+struct gpe_sim {
+    gpe_grid* grid = nullptr;
+    int dtype = GPE_C128;
+    int radius = 1;
+    double g = 0.0, n_target = 1.0;
+    double t = 0.0;
+    int kz = 16;
+    size_t csize = 16;      // bytes per complex value
+    int64_t n = 0;          // n_active
+    void* buf[4] = {nullptr, nullptr, nullptr, nullptr};  // A (psi), B, C, D in storage order
+    void* staging = nullptr;                               // canonical staging (host copies, apply_H)
+    // library-owned scratch
+    WorkRec* d_work = nullptr;
+    int32_t n_blocks = 0;
+    double* d_partials = nullptr;
+    double* d_sums = nullptr;   // [NACC] + scale at [NACC]
+    int64_t launches = 0;
+    bool counted = false;   // registered in grid->n_sims
+    // stage timing
+    bool timing = false;
+    std::vector<cudaEvent_t> ev[4];  // pairs (start, stop) per stage
+    size_t ev_used[4] = {0, 0, 0, 0};
+};
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+int cuda_fail(cudaError_t e, const char* what) {
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return GPE_ERR_CUDA;
+}
+#define CU(call)                                           \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+#define KL(call)                                                       \
+    do {                                                               \
+        int e__ = (call);                                              \
+        if (e__ != 0) return cuda_fail((cudaError_t)e__, #call);       \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+size_t buf_bytes(int64_t n, int dtype) { return align_up((size_t)(n > 0 ? n : 1) * (dtype == GPE_C128 ? 16 : 8), 256); }
+
+PotDev pot_dev(const gpe_sim* s, double t) {
+    const GridHost& h = s->grid->h;
+    PotDev p;
+    p.kind = h.pot.kind;
+    p.nx = h.box.nx; p.ny = h.box.ny; p.nz = h.box.nz;
+    p.h = h.box.h; p.cx = h.box.center[0]; p.cy = h.box.center[1]; p.cz = h.box.center[2];
+    p.ax = h.pot.ax; p.ay = h.pot.ay; p.az = h.pot.az;
+    p.delta = delta_of_t(h.pot, t);
+    p.omega = h.pot.omega;
+    return p;
+}
+
+// Split the grid's work items into pieces of at most kz planes and upload them.
+int build_work(gpe_sim* s) {
+    const GridHost& h = s->grid->h;
+    std::vector<WorkRec> recs;
+    const int kz = s->kz;
+    for (int64_t wi = 0; wi < h.n_work(); ++wi) {
+        const int32_t k = h.wi_tile[wi];
+        const int z0 = h.wi_z0[wi], nz = h.wi_nz[wi];
+        const int kk = (nz + kz - 1) / kz;
+        for (int i = 0; i < kk; ++i) {
+            const int s0 = z0 + (int)(((int64_t)i * nz) / kk), s1 = z0 + (int)(((int64_t)(i + 1) * nz) / kk);
+            WorkRec r;
+            std::memset(&r, 0, sizeof(r));
+            r.ix0 = h.tile_xy[2 * k] * h.tx;
+            r.iy0 = h.tile_xy[2 * k + 1] * h.ty;
+            r.z0 = s0;
+            r.nz = s1 - s0;
+            r.eoff[0] = h.tile_entry_base[k] - h.tile_zlo[k];
+            r.zlo[0] = h.tile_zlo[k];
+            r.zhi[0] = h.tile_zhi[k];
+            for (int q = 1; q <= 4; ++q) {
+                const int32_t nb = h.tile_nbr[4 * k + q - 1];
+                if (nb >= 0) {
+                    r.eoff[q] = h.tile_entry_base[nb] - h.tile_zlo[nb];
+                    r.zlo[q] = h.tile_zlo[nb];
+                    r.zhi[q] = h.tile_zhi[nb];
+                }
+            }
+            const int64_t e0 = r.eoff[0] + s0, e1 = r.eoff[0] + s1 - 1;
+            r.pos0 = h.slab_base[e0];
+            r.npts = (int32_t)(h.slab_base[e1] + __builtin_popcountll(h.slab_mask[e1]) - r.pos0);
+            recs.push_back(r);
+        }
+    }
+    if (recs.size() > (size_t)0x7fffffff) return fail(GPE_ERR_UNSUPPORTED, "too many work pieces");
+    if (s->d_work) { cudaFree(s->d_work); s->d_work = nullptr; }
+    if (s->d_partials) { cudaFree(s->d_partials); s->d_partials = nullptr; }
+    s->n_blocks = (int32_t)recs.size();
+    const size_t nrec = recs.empty() ? 1 : recs.size();
+    cudaError_t e = cudaMalloc(&s->d_work, nrec * sizeof(WorkRec));
+    if (e == cudaErrorMemoryAllocation) return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(work records)");
+    CU(e);
+    if (!recs.empty()) CU(cudaMemcpy(s->d_work, recs.data(), recs.size() * sizeof(WorkRec), cudaMemcpyHostToDevice));
+    size_t np = std::max<size_t>(nrec, (size_t)norm_blocks(s->n));
+    e = cudaMalloc(&s->d_partials, np * NACC * sizeof(double));
+    if (e == cudaErrorMemoryAllocation) return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(partials)");
+    CU(e);
+    return GPE_OK;
+}
+
+int upload_grid(gpe_grid* g) {
+    if (g->on_device) return GPE_OK;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) return fail(GPE_ERR_CUDA, "device is not sm_100 (B200): kernels are built for sm_100a only");
+    KL(kernels_configure());
+    const GridHost& h = g->h;
+    const size_t ns = (size_t)std::max<int64_t>(h.n_slabs(), 1), na = (size_t)std::max<int64_t>(h.n_active, 1);
+    cudaError_t e = cudaMalloc(&g->d_slabs, ns * sizeof(Slab));
+    if (e == cudaErrorMemoryAllocation) return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(slabs)");
+    CU(e);
+    e = cudaMalloc(&g->d_perm, na * sizeof(int64_t));
+    if (e == cudaErrorMemoryAllocation) { cudaFree(g->d_slabs); g->d_slabs = nullptr; return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(perm)"); }
+    CU(e);
+    std::vector<Slab> slabs((size_t)h.n_slabs());
+    for (int64_t k = 0; k < h.n_slabs(); ++k) { slabs[k].mask = h.slab_mask[k]; slabs[k].base = h.slab_base[k]; }
+    if (!slabs.empty()) CU(cudaMemcpy(g->d_slabs, slabs.data(), slabs.size() * sizeof(Slab), cudaMemcpyHostToDevice));
+    if (h.n_active > 0)
+        CU(cudaMemcpy(g->d_perm, h.storage_to_canonical.data(), (size_t)h.n_active * sizeof(int64_t), cudaMemcpyHostToDevice));
+    g->device = dev;
+    g->on_device = true;
+    return GPE_OK;
+}
+
+StageParams base_params(const gpe_sim* s, double t) {
+    StageParams p;
+    std::memset(&p, 0, sizeof(p));
+    p.slabs = s->grid->d_slabs;
+    p.work = s->d_work;
+    p.n_work = s->n_blocks;
+    p.kz = s->kz;
+    p.pot = pot_dev(s, t);
+    p.g = s->g;
+    p.partials = s->d_partials;
+    p.scale_in = s->d_sums + NACC;
+    return p;
+}
+
+int stage(gpe_sim* s, int mode, double t, double ca, const void* in, const void* aux, void* out1, void* out2,
+          void* stream, int timed_slot = -1) {
+    StageParams p = base_params(s, t);
+    p.ca = ca; p.in = in; p.aux = aux; p.out1 = out1; p.out2 = out2;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (s->timing && timed_slot >= 0) {
+        auto& v = s->ev[timed_slot];
+        size_t& u = s->ev_used[timed_slot];
+        while (v.size() < u + 2) {
+            cudaEvent_t e;
+            CU(cudaEventCreate(&e));
+            v.push_back(e);
+        }
+        CU(cudaEventRecord(v[u], st));
+        KL(launch_stage(s->dtype, s->radius, mode, p, stream));
+        CU(cudaEventRecord(v[u + 1], st));
+        u += 2;
+    } else {
+        KL(launch_stage(s->dtype, s->radius, mode, p, stream));
+    }
+    if (s->n_blocks > 0) s->launches += 1;
+    return GPE_OK;
+}
+
+int rk4_step(gpe_sim* s, double t, double dt, void* stream) {
+    void *A = s->buf[0], *B = s->buf[1], *C = s->buf[2], *D = s->buf[3];
+    int rc;
+    // PAPER.md:276-281 Eq. A6-A7 with a*, b* of Eq. A10-A11 (RK4); b* = [-1/3, 1/3, 2/3, 1/3]
+    if ((rc = stage(s, MODE_S1, t, 0.5 * dt, A, nullptr, B, nullptr, stream, 0))) return rc;            // y2
+    if ((rc = stage(s, MODE_S2, t + 0.5 * dt, 0.5 * dt, B, A, C, D, stream, 1))) return rc;             // y3, p
+    if ((rc = stage(s, MODE_S3, t + 0.5 * dt, dt, C, A, B, nullptr, stream, 2))) return rc;             // y4
+    if ((rc = stage(s, MODE_S4, t + dt, dt / 6.0, B, D, A, nullptr, stream, 3))) return rc;             // y_new
+    return GPE_OK;
+}
+
+int sums_to_host(gpe_sim* s, double out[NACC], void* stream) {
+    CU(cudaMemcpyAsync(out, s->d_sums, NACC * sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    return GPE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* gpe_last_error(void) { return g_err.c_str(); }
+
+int gpe_grid_create(const gpe_box* box, const gpe_potential* pot, double v_cut, int halo_width, gpe_grid** out) {
+    if (!box || !pot || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    gpe_grid* g = new (std::nothrow) gpe_grid();
+    if (!g) return fail(GPE_ERR_OUT_OF_MEMORY, "host allocation");
+    std::string err;
+    int rc = build_layout_from_potential(*box, *pot, v_cut, halo_width, &g->h, &err);
+    if (rc) { delete g; return fail(rc, err); }
+    *out = g;
+    return GPE_OK;
+}
+
+int gpe_grid_create_from_indices(const gpe_box* box, const gpe_potential* pot, const int64_t* active_host, int64_t n,
+                                 int halo_width, gpe_grid** out) {
+    if (!box || !pot || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    gpe_grid* g = new (std::nothrow) gpe_grid();
+    if (!g) return fail(GPE_ERR_OUT_OF_MEMORY, "host allocation");
+    std::string err;
+    int rc = build_layout_from_indices(*box, *pot, active_host, n, halo_width, &g->h, &err);
+    if (rc) { delete g; return fail(rc, err); }
+    *out = g;
+    return GPE_OK;
+}
+
+int gpe_grid_destroy(gpe_grid* g) {
+    if (!g) return GPE_OK;
+    if (g->n_sims > 0) return fail(GPE_ERR_STATE, "destroy the sims created on this grid first");
+    if (g->d_slabs) cudaFree(g->d_slabs);
+    if (g->d_perm) cudaFree(g->d_perm);
+    delete g;
+    return GPE_OK;
+}
+
+int gpe_grid_num_active(const gpe_grid* g, int64_t* out) {
+    if (!g || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    *out = g->h.n_active;
+    return GPE_OK;
+}
+
+int gpe_grid_num_stored(gpe_grid* g, int64_t* out) {
+    if (!g || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    try {
+        build_stored_indices(&g->h);
+    } catch (const std::bad_alloc&) {
+        return fail(GPE_ERR_OUT_OF_MEMORY, "host allocation (stored indices)");
+    }
+    *out = (int64_t)g->h.stored_idx.size();
+    return GPE_OK;
+}
+
+int gpe_grid_layout_info(const gpe_grid* g, gpe_layout_info* out) {
+    if (!g || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    out->tx = g->h.tx; out->ty = g->h.ty; out->zt = g->h.zt; out->halo_width = g->h.halo_width;
+    out->n_active = g->h.n_active;
+    out->n_tiles = g->h.n_tiles();
+    out->n_slabs = g->h.n_slabs();
+    out->n_work = g->h.n_work();
+    return GPE_OK;
+}
+
+int gpe_grid_active_indices(const gpe_grid* g, int64_t* out_host) {
+    if (!g || !out_host) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (g->h.n_active) std::memcpy(out_host, g->h.active_idx.data(), (size_t)g->h.n_active * sizeof(int64_t));
+    return GPE_OK;
+}
+
+int gpe_grid_stored_indices(gpe_grid* g, int64_t* out_host) {
+    if (!g || !out_host) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    try {
+        build_stored_indices(&g->h);
+    } catch (const std::bad_alloc&) {
+        return fail(GPE_ERR_OUT_OF_MEMORY, "host allocation (stored indices)");
+    }
+    if (!g->h.stored_idx.empty()) std::memcpy(out_host, g->h.stored_idx.data(), g->h.stored_idx.size() * sizeof(int64_t));
+    return GPE_OK;
+}
+
+int gpe_grid_layout_tables(const gpe_grid* g, const gpe_layout_tables* o) {
+    if (!g || !o) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    const GridHost& h = g->h;
+    auto cp = [](void* dst, const void* src, size_t bytes) { if (dst && bytes) std::memcpy(dst, src, bytes); };
+    cp(o->tile_xy, h.tile_xy.data(), h.tile_xy.size() * sizeof(int32_t));
+    cp(o->tile_zlo, h.tile_zlo.data(), h.tile_zlo.size() * sizeof(int32_t));
+    cp(o->tile_zhi, h.tile_zhi.data(), h.tile_zhi.size() * sizeof(int32_t));
+    cp(o->tile_entry_base, h.tile_entry_base.data(), h.tile_entry_base.size() * sizeof(int64_t));
+    cp(o->tile_nbr, h.tile_nbr.data(), h.tile_nbr.size() * sizeof(int32_t));
+    cp(o->slab_mask, h.slab_mask.data(), h.slab_mask.size() * sizeof(uint64_t));
+    cp(o->slab_base, h.slab_base.data(), h.slab_base.size() * sizeof(int64_t));
+    cp(o->wi_tile, h.wi_tile.data(), h.wi_tile.size() * sizeof(int32_t));
+    cp(o->wi_z0, h.wi_z0.data(), h.wi_z0.size() * sizeof(int32_t));
+    cp(o->wi_nz, h.wi_nz.data(), h.wi_nz.size() * sizeof(int32_t));
+    cp(o->storage_to_canonical, h.storage_to_canonical.data(), h.storage_to_canonical.size() * sizeof(int64_t));
+    return GPE_OK;
+}
+
+int gpe_sim_state_bytes(const gpe_grid* g, int dtype, size_t* out) {
+    if (!g || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (dtype != GPE_C64 && dtype != GPE_C128) return fail(GPE_ERR_INVALID_ARG, "unknown dtype");
+    *out = 5 * buf_bytes(g->h.n_active, dtype);
+    return GPE_OK;
+}
+
+int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_target, void* dev_state,
+                   size_t state_bytes, void* stream, gpe_sim** out) {
+    if (!g || !dev_state || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (dtype != GPE_C64 && dtype != GPE_C128) return fail(GPE_ERR_INVALID_ARG, "unknown dtype");
+    if (stencil != 7 && stencil != 13) return fail(GPE_ERR_INVALID_ARG, "stencil must be 7 or 13");
+    if (!(n_target > 0.0)) return fail(GPE_ERR_INVALID_ARG, "n_target must be > 0");
+    const int radius = stencil == 7 ? 1 : 2;
+    if (g->h.tx != 8 || g->h.ty != 8) return fail(GPE_ERR_UNSUPPORTED, "kernels need 8x8 column tiles");
+    if (g->h.halo_width < radius) return fail(GPE_ERR_UNSUPPORTED, "grid halo_width is smaller than the stencil radius");
+    if (((uintptr_t)dev_state & 255) != 0) return fail(GPE_ERR_INVALID_ARG, "dev_state must be 256-byte aligned");
+    const size_t bb = buf_bytes(g->h.n_active, dtype);
+    if (state_bytes < 5 * bb) return fail(GPE_ERR_INVALID_ARG, "state_bytes too small (see gpe_sim_state_bytes)");
+    int rc = upload_grid(g);
+    if (rc) return rc;
+    gpe_sim* s = new (std::nothrow) gpe_sim();
+    if (!s) return fail(GPE_ERR_OUT_OF_MEMORY, "host allocation");
+    s->grid = g;
+    s->dtype = dtype;
+    s->radius = radius;
+    s->g = g_int;
+    s->n_target = n_target;
+    s->csize = dtype == GPE_C128 ? 16 : 8;
+    s->n = g->h.n_active;
+    s->kz = 16;
+    for (int k = 0; k < 4; ++k) s->buf[k] = (char*)dev_state + k * bb;
+    s->staging = (char*)dev_state + 4 * bb;
+    cudaError_t e = cudaMalloc(&s->d_sums, (NACC + 1) * sizeof(double));
+    if (e != cudaSuccess) { delete s; return e == cudaErrorMemoryAllocation ? fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc") : cuda_fail(e, "cudaMalloc"); }
+    rc = build_work(s);
+    if (rc) { gpe_sim_destroy(s); return rc; }
+    cudaStream_t st = (cudaStream_t)stream;
+    e = cudaMemsetAsync(dev_state, 0, 5 * bb, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_sums, 0, (NACC + 1) * sizeof(double), st);
+    if (e == cudaSuccess) e = (cudaError_t)launch_set_scalar(s->d_sums + NACC, 1.0, stream);
+    if (e != cudaSuccess) { gpe_sim_destroy(s); return cuda_fail(e, "state initialisation"); }
+    g->n_sims += 1;
+    s->counted = true;
+    s->launches += 1;
+    *out = s;
+    return GPE_OK;
+}
+
+int gpe_sim_destroy(gpe_sim* s) {
+    if (!s) return GPE_OK;
+    if (s->d_work) cudaFree(s->d_work);
+    if (s->d_partials) cudaFree(s->d_partials);
+    if (s->d_sums) cudaFree(s->d_sums);
+    for (int k = 0; k < 4; ++k)
+        for (cudaEvent_t e : s->ev[k]) cudaEventDestroy(e);
+    if (s->counted && s->grid && s->grid->n_sims > 0) s->grid->n_sims -= 1;
+    delete s;
+    return GPE_OK;
+}
+
+int gpe_set_psi(gpe_sim* s, const void* dev_psi_canonical, void* stream) {
+    if (!s || (!dev_psi_canonical && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    KL(launch_pack(s->dtype, dev_psi_canonical, s->buf[0], s->grid->d_perm, s->n, stream));
+    if (s->n > 0) s->launches += 1;
+    return GPE_OK;
+}
+
+int gpe_get_psi(gpe_sim* s, void* dev_psi_canonical, void* stream) {
+    if (!s || (!dev_psi_canonical && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    KL(launch_unpack(s->dtype, s->buf[0], dev_psi_canonical, s->grid->d_perm, s->n, stream));
+    if (s->n > 0) s->launches += 1;
+    return GPE_OK;
+}
+
+int gpe_set_psi_host(gpe_sim* s, const void* host_psi_canonical, void* stream) {
+    if (!s || (!host_psi_canonical && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (s->n == 0) return GPE_OK;
+    CU(cudaMemcpyAsync(s->staging, host_psi_canonical, (size_t)s->n * s->csize, cudaMemcpyHostToDevice, (cudaStream_t)stream));
+    int rc = gpe_set_psi(s, s->staging, stream);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    return GPE_OK;
+}
+
+int gpe_get_psi_host(gpe_sim* s, void* host_psi_canonical, void* stream) {
+    if (!s || (!host_psi_canonical && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (s->n == 0) return GPE_OK;
+    int rc = gpe_get_psi(s, s->staging, stream);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(host_psi_canonical, s->staging, (size_t)s->n * s->csize, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    return GPE_OK;
+}
+
+int gpe_set_time(gpe_sim* s, double t) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (!std::isfinite(t)) return fail(GPE_ERR_INVALID_ARG, "t must be finite");
+    s->t = t;
+    return GPE_OK;
+}
+
+int gpe_get_time(const gpe_sim* s, double* t) {
+    if (!s || !t) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    *t = s->t;
+    return GPE_OK;
+}
+
+int gpe_apply_H(gpe_sim* s, double t, const void* dev_in_canonical, void* dev_out_canonical, void* stream) {
+    if (!s || ((!dev_in_canonical || !dev_out_canonical) && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (s->n == 0) return GPE_OK;
+    const char* a = (const char*)dev_in_canonical;
+    const char* b = (const char*)dev_out_canonical;
+    const size_t bytes = (size_t)s->n * s->csize;
+    if (a < b + bytes && b < a + bytes) return fail(GPE_ERR_INVALID_ARG, "in and out overlap");
+    // scratch: C holds the packed input, D the packed result; the sim's psi (A) is untouched
+    KL(launch_pack(s->dtype, dev_in_canonical, s->buf[2], s->grid->d_perm, s->n, stream));
+    s->launches += 1;
+    int rc = stage(s, MODE_APPLY, t, 0.0, s->buf[2], nullptr, s->buf[3], nullptr, stream);
+    if (rc) return rc;
+    KL(launch_unpack(s->dtype, s->buf[3], dev_out_canonical, s->grid->d_perm, s->n, stream));
+    s->launches += 1;
+    return GPE_OK;
+}
+
+int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
+    const double t0 = s->t;
+    for (int64_t n = 0; n < nsteps; ++n) {
+        int rc = rk4_step(s, t0 + (double)n * dt, dt, stream);
+        if (rc) return rc;
+    }
+    s->t = t0 + (double)nsteps * dt;
+    return GPE_OK;
+}
+
+int gpe_step_rk4(gpe_sim* s, double dt, void* stream) { return gpe_run_rk4(s, dt, 1, stream); }
+
+int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
+    if (s->n == 0 || nsteps == 0) return GPE_OK;
+    const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;
+    for (int64_t n = 0; n < nsteps; ++n) {
+        int rc = stage(s, MODE_IMAG, s->t, dt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
+        if (rc) return rc;
+        KL(launch_finalize(s->d_partials, s->n_blocks, s->d_sums, s->d_sums + NACC, s->n_target, h3, stream));
+        s->launches += 1;
+        std::swap(s->buf[0], s->buf[1]);
+    }
+    // flush the lazy scale so that every other call sees a normalised state
+    KL(launch_scale(s->dtype, s->buf[0], s->n, s->d_sums + NACC, stream));
+    KL(launch_set_scalar(s->d_sums + NACC, 1.0, stream));
+    s->launches += 2;
+    return GPE_OK;
+}
+
+int gpe_imag_step(gpe_sim* s, double dt, void* stream) { return gpe_run_imag(s, dt, 1, stream); }
+
+int gpe_norm(gpe_sim* s, double* out_host, void* stream) {
+    if (!s || !out_host) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;
+    if (s->n == 0) { *out_host = 0.0; return GPE_OK; }
+    KL(launch_norm_partials(s->dtype, s->buf[0], s->n, s->d_partials, stream));
+    KL(launch_finalize(s->d_partials, norm_blocks(s->n), s->d_sums, nullptr, s->n_target, h3, stream));
+    s->launches += 2;
+    double sums[NACC];
+    int rc = sums_to_host(s, sums, stream);
+    if (rc) return rc;
+    const double v = h3 * sums[0];
+    if (!std::isfinite(v)) return fail(GPE_ERR_STATE, "norm is not finite");
+    *out_host = v;
+    return GPE_OK;
+}
+
+int gpe_energy(gpe_sim* s, gpe_energy_out* o, void* stream) {
+    if (!s || !o) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;
+    if (s->n == 0) return fail(GPE_ERR_STATE, "empty grid has no energy");
+    int rc = stage(s, MODE_ENERGY, s->t, 0.0, s->buf[0], nullptr, nullptr, nullptr, stream);
+    if (rc) return rc;
+    KL(launch_finalize(s->d_partials, s->n_blocks, s->d_sums, nullptr, s->n_target, h3, stream));
+    s->launches += 1;
+    double sums[NACC];
+    rc = sums_to_host(s, sums, stream);
+    if (rc) return rc;
+    gpe_energy_out r;
+    r.kin = h3 * sums[0];
+    r.pot = h3 * sums[1];
+    r.inter = h3 * 0.5 * s->g * sums[2];
+    r.norm = h3 * sums[3];
+    r.total = r.kin + r.pot + r.inter;
+    r.mu = (r.kin + r.pot + 2.0 * r.inter) / r.norm;
+    if (!std::isfinite(r.mu) || !(r.norm > 0.0)) return fail(GPE_ERR_STATE, "state has zero or non-finite norm");
+    *o = r;
+    return GPE_OK;
+}
+
+int gpe_sim_kernel_launches(const gpe_sim* s, int64_t* out) {
+    if (!s || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    *out = s->launches;
+    return GPE_OK;
+}
+
+int gpe_sim_time_stages(gpe_sim* s, int on) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    s->timing = on != 0;
+    for (int k = 0; k < 4; ++k) s->ev_used[k] = 0;
+    return GPE_OK;
+}
+
+int gpe_sim_stage_time_ms(gpe_sim* s, double ms_out[4], int64_t count_out[4]) {
+    if (!s || !ms_out || !count_out) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    for (int k = 0; k < 4; ++k) {
+        double acc = 0.0;
+        for (size_t u = 0; u + 1 < s->ev_used[k]; u += 2) {
+            CU(cudaEventSynchronize(s->ev[k][u + 1]));
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, s->ev[k][u], s->ev[k][u + 1]));
+            acc += ms;
+        }
+        ms_out[k] = acc;
+        count_out[k] = (int64_t)(s->ev_used[k] / 2);
+        s->ev_used[k] = 0;
+    }
+    return GPE_OK;
+}
+
+int gpe_sim_set_planes_per_block(gpe_sim* s, int kz) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (kz < 1 || kz > 32) return fail(GPE_ERR_INVALID_ARG, "planes per block must be in 1..32");
+    if (stage_smem_bytes(s->dtype, s->radius, kz) > 200 * 1024) return fail(GPE_ERR_INVALID_ARG, "tile does not fit shared memory");
+    CU(cudaDeviceSynchronize());
+    s->kz = kz;
+    return build_work(s);
+}
+
+}  // extern "C"

@@ -1,0 +1,129 @@
+// Internal declarations shared by the host layout builder (gpe_layout.cpp), the C-ABI glue
+// (gpe_api.cu) and the kernels (gpe_kernels.cu).  Not part of the public boundary (include/gpe.h).
+#pragma once
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "gpe.h"
+
+namespace gpe {
+
+// ---------------------------------------------------------------------------------------------
+// Host-side layout (prior art PAPER.md:81-85)
+// ---------------------------------------------------------------------------------------------
+struct GridHost {
+    gpe_box box{};
+    gpe_potential pot{};
+    double v_cut = 0.0;
+    int halo_width = 0;
+    int tx = 8, ty = 8, zt = 32;
+    int ntx = 0, nty = 0;
+    int64_t n_active = 0;
+
+    std::vector<int32_t> tile_xy;          // [n_tiles][2]
+    std::vector<int32_t> tile_zlo, tile_zhi;
+    std::vector<int64_t> tile_entry_base;  // [n_tiles]
+    std::vector<int32_t> tile_nbr;         // [n_tiles][4]
+    std::vector<uint64_t> slab_mask;       // [n_slabs]
+    std::vector<int64_t> slab_base;        // [n_slabs]
+    std::vector<int32_t> wi_tile, wi_z0, wi_nz;
+    std::vector<int64_t> storage_to_canonical;  // [n_active]
+    std::vector<int64_t> active_idx;            // [n_active]
+
+    bool stored_ready = false;
+    std::vector<int64_t> stored_idx;
+
+    int64_t n_tiles() const { return (int64_t)tile_zlo.size(); }
+    int64_t n_slabs() const { return (int64_t)slab_mask.size(); }
+    int64_t n_work() const { return (int64_t)wi_tile.size(); }
+};
+
+// Builders: return GPE_OK or an error code and fill `err`.
+int build_layout_from_potential(const gpe_box& box, const gpe_potential& pot, double v_cut, int halo_width,
+                                GridHost* out, std::string* err);
+int build_layout_from_indices(const gpe_box& box, const gpe_potential& pot, const int64_t* active, int64_t n,
+                              int halo_width, GridHost* out, std::string* err);
+void build_stored_indices(GridHost* g);
+
+// Delta(t) of the linear ramp (R16); same formula as the oracle's, one rounding each.
+double delta_of_t(const gpe_potential& pot, double t);
+
+// ---------------------------------------------------------------------------------------------
+// Device-side tables and kernel parameters
+// ---------------------------------------------------------------------------------------------
+struct Slab {                // one z-plane of one tile
+    unsigned long long mask; // bit lx*8+ly set iff the point is in M
+    long long base;          // storage position of the slab's first lane
+};
+
+// One thread block's worth of work: nz consecutive planes of one tile (a piece of a work item).
+// eoff[q] + zp = slab entry of plane zp in tile q (0 = own, 1..4 = -x,+x,-y,+y), valid for
+// zlo[q] <= zp < zhi[q] (zlo = zhi = 0 when the neighbour tile is absent).
+struct alignas(16) WorkRec {
+    int32_t ix0, iy0;   // box index of the tile's (lx,ly) = (0,0) column
+    int32_t z0, nz;
+    long long eoff[5];
+    int32_t zlo[5];
+    int32_t zhi[5];
+    long long pos0;     // storage position of the first point of the piece
+    int32_t npts;       // points in the piece (contiguous in storage from pos0)
+    int32_t pad[5];
+};
+static_assert(sizeof(WorkRec) == 128, "WorkRec layout");
+
+struct PotDev {
+    int32_t kind;
+    int32_t nx, ny, nz;
+    double h, cx, cy, cz;
+    double ax, ay, az;
+    double delta;   // Delta at the stage time (host-computed, R16)
+    double omega;
+};
+
+enum Mode : int {
+    MODE_APPLY = 0,  // out1 = H c
+    MODE_S1 = 1,     // out1 = c + ca * f(c)                        f(c) = -i H c
+    MODE_S2 = 2,     // out1 = aux + ca * f(c); out2 = -1/3 aux + 1/3 c + 2/3 out1
+    MODE_S3 = 3,     // out1 = aux + ca * f(c)
+    MODE_S4 = 4,     // out1 = aux + 1/3 c + ca * f(c)
+    MODE_IMAG = 5,   // psi = scale * c; out1 = psi - ca * H psi; partial sum of |out1|^2
+    MODE_ENERGY = 6  // partial sums of Re(conj(c) T c), V|c|^2, |c|^4, |c|^2
+};
+constexpr int NACC = 4;           // accumulators per block in the partial-sum array
+constexpr int STAGE_THREADS = 256;
+
+struct StageParams {
+    const Slab* slabs;
+    const WorkRec* work;
+    int32_t n_work;
+    int32_t kz;            // max planes per block (smem tile is sized for it)
+    PotDev pot;
+    double g;
+    double ca;             // stage coefficient (dt/2, dt, dt/6, or dt of the imaginary step)
+    const void* in;        // array the stencil is applied to (storage order)
+    const void* aux;       // y0 or p (storage order) or null
+    void* out1;
+    void* out2;
+    const double* scale_in;  // MODE_IMAG: device scalar multiplying `in` on load (lazy renormalisation)
+    double* partials;        // MODE_IMAG / MODE_ENERGY: [n_work][NACC] block partial sums
+};
+
+// Launchers (gpe_kernels.cu).  dtype: GPE_C64 / GPE_C128; radius 1 or 2.  Return cudaError_t as int.
+int launch_stage(int dtype, int radius, int mode, const StageParams& p, void* stream);
+size_t stage_smem_bytes(int dtype, int radius, int kz);
+int launch_pack(int dtype, const void* canonical, void* storage, const int64_t* perm, int64_t n, void* stream);
+int launch_unpack(int dtype, const void* storage, void* canonical, const int64_t* perm, int64_t n, void* stream);
+// partials[b*NACC + 0] = sum over the block's contiguous chunk of |psi|^2; nblk = norm_blocks(n)
+int norm_blocks(int64_t n);
+int launch_norm_partials(int dtype, const void* storage, int64_t n, double* partials, void* stream);
+// out[k] = sum_b partials[b*NACC + k] in a fixed order (k < NACC); if scale_out != null also writes
+// scale_out[0] = sqrt(n_target / (h3 * out[0]))
+int launch_finalize(const double* partials, int64_t nblk, double* out, double* scale_out,
+                    double n_target, double h3, void* stream);
+int launch_scale(int dtype, void* storage, int64_t n, const double* scale, void* stream);
+int launch_set_scalar(double* dst, double v, void* stream);
+int kernels_configure();  // sets max dynamic shared memory attributes once; returns cudaError_t
+
+}  // namespace gpe

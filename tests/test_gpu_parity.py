@@ -1,0 +1,169 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's north_star: max relative error (R10:
+max|a-b| / max|b|) 1e-12 per operator application and 1e-9 after 1000 steps in complex128; 1e-5 and 1e-3
+in complex64 (the complex64 result is compared against the complex128 oracle fed the fp32-rounded input)."""
+import numpy as np
+import pytest
+
+import gpe_inputs as I
+from helpers import RADIUS, oracle_objs, rel_max
+from oracle import c_oracle as CO
+from oracle import gpe_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+TOL_APPLY = {"complex128": 1e-12, "complex64": 1e-5}
+TOL_STEPS = {"complex128": 1e-9, "complex64": 1e-3}
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2603_05447_b200 as P
+    return P
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _dev(x, dtype):
+    torch = _torch()
+    return torch.from_numpy(np.ascontiguousarray(x)).to("cuda:0").to(getattr(torch, dtype))
+
+
+def _make(P, w, active=None, dtype=None):
+    box, pot, act = oracle_objs(w, active)
+    grid = P.Grid.from_workload(w, active=active)
+    assert np.array_equal(grid.active_indices(), act)
+    sim = P.Sim(grid, dtype or w.dtype, w.stencil, w.g)
+    return box, pot, act, grid, sim
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+@pytest.mark.parametrize("stencil", [7, 13])
+@pytest.mark.parametrize("kz", [16, 5, 32])
+def test_apply_H_small_shell(P, stencil, dtype, kz):
+    w = I.small_shell(40, stencil, dtype).with_(delta0=14.0, delta1=22.0, t_ramp=0.5)
+    box, pot, act, grid, sim = _make(P, w)
+    sim.set_planes_per_block(kz)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.random_psi(7, act.size).astype(sim.npdtype)
+    for t in (0.0, 0.3, 2.0):
+        got = sim.apply_H(t, _dev(psi, dtype)).cpu().numpy()
+        ref = O.apply_H(og, pot, w.g, t, psi.astype(np.complex128), stencil)
+        assert rel_max(got, ref) < TOL_APPLY[dtype]
+
+
+@pytest.mark.parametrize("dims,p,seed", [((9, 7, 11), 0.4, 3), ((17, 16, 40), 0.15, 4), ((8, 8, 70), 0.9, 5),
+                                         ((6, 6, 6), 1.1, 6), ((19, 21, 37), 0.6, 8)])
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_apply_H_random_masks(P, dims, p, seed, stencil):
+    """Random masks (holes everywhere, box faces touched) and the full 6^3 box."""
+    nx, ny, nz = dims
+    w = I.Workload(name="rnd", nx=nx, ny=ny, nz=nz, h=0.3, kind=I.DRESSED, ax=1.0, ay=0.7, az=1.2, delta0=2.0,
+                   delta1=2.0, omega=1.5, stencil=stencil, g=3.0)
+    act = I.random_mask_lin(seed, nx, ny, nz, p)
+    box, pot, act, grid, sim = _make(P, w, active=act)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.random_psi(seed + 100, act.size)
+    got = sim.apply_H(0.1, _dev(psi, "complex128")).cpu().numpy()
+    assert rel_max(got, O.apply_H(og, pot, w.g, 0.1, psi, stencil)) < 1e-12
+
+
+def test_single_point_and_empty(P):
+    w = I.Workload(name="one", nx=5, ny=4, nz=3, h=0.5, kind=I.HARMONIC, stencil=13, g=2.0)
+    box, pot, act, grid, sim = _make(P, w, active=np.array([17], np.int64))
+    og = O.SparseGrid(box, act, 2)
+    psi = np.array([0.3 - 0.8j])
+    got = sim.apply_H(0.0, _dev(psi, "complex128")).cpu().numpy()
+    assert rel_max(got, O.apply_H(og, pot, w.g, 0.0, psi, 13)) < 1e-12
+    sim.set_psi_host(psi)
+    sim.run_rk4(1e-3, 3)
+    assert rel_max(sim.get_psi_host(), O.run_rk4(og, pot, w.g, 0.0, 1e-3, 3, psi, 13)) < 1e-12
+    # empty grid: every call is a no-op
+    grid0 = P.Grid.from_workload(w.with_(v_cut=-1.0))
+    sim0 = P.Sim(grid0, "complex128", 13, 1.0)
+    sim0.run_rk4(1e-3, 2)
+    sim0.run_imag(1e-3, 2)
+    assert sim0.norm() == 0.0 and sim0.get_psi_host().size == 0
+
+
+def test_set_get_roundtrip_and_norm(P):
+    w = I.small_shell(40, 13)
+    box, pot, act, grid, sim = _make(P, w)
+    psi = I.make_psi0(w, act)
+    sim.set_psi_host(psi)
+    assert np.array_equal(sim.get_psi_host(), psi)
+    d = _dev(psi, "complex128")
+    sim.set_psi(d)
+    assert np.array_equal(sim.get_psi().cpu().numpy(), psi)
+    og = O.SparseGrid(box, act, 2)
+    assert abs(sim.norm() - O.norm(og, psi)) < 1e-13
+    assert sim.norm() == sim.norm()  # fixed summation order: bit-reproducible
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_rk4_small_shell_with_ramp(P, stencil, dtype):
+    """RK4 stage-state form (PAPER.md Eq. A6-A7, A10-A11) against the textbook k1..k4 oracle with a
+    time-ramped potential (stage times t, t+dt/2, t+dt/2, t+dt)."""
+    w = I.small_shell(40, stencil, dtype).with_(delta0=14.0, delta1=22.0, t_ramp=0.02)
+    box, pot, act, grid, sim = _make(P, w)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    sim.time = 0.005
+    sim.run_rk4(w.dt, 4)
+    sim.step_rk4(w.dt)
+    assert abs(sim.time - (0.005 + 5 * w.dt)) < 1e-15
+    ref = O.run_rk4(og, pot, w.g, 0.005, w.dt, 5, psi.astype(np.complex128), stencil)
+    assert rel_max(sim.get_psi_host(), ref) < (1e-12 if dtype == "complex128" else 1e-5)
+
+
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_imag_and_energy_small_shell(P, stencil):
+    w = I.small_shell(40, stencil)
+    box, pot, act, grid, sim = _make(P, w)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.make_psi0(w, act)
+    sim.set_psi_host(psi)
+    e = sim.energy()
+    ref = O.energy(og, pot, w.g, 0.0, psi, stencil)
+    for k in ref:
+        assert abs(e[k] - ref[k]) <= 1e-12 * max(1.0, abs(ref[k])), k
+    sim.run_imag(1e-3, 9)
+    sim.imag_step(1e-3)
+    ref = O.run_imag(og, pot, w.g, 0.0, 1e-3, 10, psi, stencil)
+    assert rel_max(sim.get_psi_host(), ref) < 1e-12
+    assert abs(sim.norm() - 1.0) < 1e-12
+    e2 = sim.energy()
+    assert e2["total"] < e["total"]  # imaginary time lowers the energy
+
+
+def test_config1_100_and_1000_steps(P):
+    """BASELINE configs[0]: 48^3 harmonic trap, 7-pt, g=100, complex128; 100 steps and the 1e-9 bound
+    after 1000 steps (C oracle: explicit loops, textbook RK4)."""
+    w = I.config1()
+    box, pot, act, grid, sim = _make(P, w)
+    co = CO.COracle(box, pot, act, w.stencil)
+    psi = I.make_psi0(w, act)
+    sim.set_psi_host(psi)
+    sim.run_rk4(w.dt, 100)
+    ref = co.run_rk4(w.g, 0.0, w.dt, 100, psi)
+    assert rel_max(sim.get_psi_host(), ref) < 1e-11
+    sim.run_rk4(w.dt, 900)
+    ref = co.run_rk4(w.g, 100 * w.dt, w.dt, 900, ref)
+    assert rel_max(sim.get_psi_host(), ref) < 1e-9
+    assert abs(sim.norm() - co.norm(ref)) < 1e-11
+
+
+def test_config1_complex64_1000_steps(P):
+    w = I.config1().with_(dtype="complex64")
+    box, pot, act, grid, sim = _make(P, w)
+    co = CO.COracle(box, pot, act, w.stencil)
+    psi = I.make_psi0(w, act).astype(np.complex64)
+    sim.set_psi_host(psi)
+    sim.run_rk4(w.dt, 1000)
+    ref = co.run_rk4(w.g, 0.0, w.dt, 1000, psi.astype(np.complex128))
+    assert rel_max(sim.get_psi_host(), ref) < 1e-3

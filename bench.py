@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""Benchmark of the sparse-grid Gross-Pitaevskii hot path (BASELINE.json metric: active-point RK4 stage
+updates per second, with the achieved fraction of the HBM roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A "step" is one RK4 time step (the four fused stage kernels S1-S4 = stencil + V(r,t) + nonlinear term +
+Runge-Kutta combination) through the C ABI (gpe_run_rk4) on the workload named in `config.workload`; the
+default is BASELINE configs[3], the 1024^3 anisotropic ellipsoidal bubble in complex128 with the 13-point
+stencil ("the largest shell workload" the north_star quotes the target on).  The other rows of the path
+(layout build, imaginary-time step, reductions, pack/unpack) are timed in the same run and reported under
+"extra".  One JSON line is printed by rank 0.  See DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gpe_inputs as I  # noqa: E402
+
+METRIC = "active_point_rk4_stage_updates_per_s"
+UNIT = "stage_updates/s"
+# algorithmic HBM elements per active point of the four stage kernels
+STAGE_ELEMS = (2, 4, 3, 3)
+
+
+def workloads():
+    return {
+        "cfg4_c128": I.config4("complex128"),
+        "cfg4_c64": I.config4("complex64"),
+        "cfg2": I.config2().with_(dt=1e-4),
+        "cfg3a": I.config3(True),
+        "cfg3b": I.config3(False),
+        "cfg1": I.config1(),
+        "cfg5_dense_c128": I.config5_dense(512, 13, "complex128"),
+        "cfg5_1e7_c128": I.config5_shell(1e7, 24, 13, "complex128", 4),
+        "cfg5_1e8_c128": I.config5_shell(1e8, 24, 13, "complex128", 6),
+        "small": I.small_shell(40, 13),
+    }
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def recorded_traffic(name, dtype_key):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, if one was recorded."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(name, {}).get(dtype_key)
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            self.nv = nv
+            self.h = nv.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {}
+        for n in dir(nv):
+            if n.startswith("nvmlClocksEventReason") or n.startswith("nvmlClocksThrottleReason"):
+                v = getattr(nv, n)
+                if isinstance(v, int) and v:
+                    names[v] = n.replace("nvmlClocksEventReason", "").replace("nvmlClocksThrottleReason", "")
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit and bit & (bit - 1) == 0:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def start(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        med = statistics.median(self.samples) if self.samples else None
+        bad = {"HwSlowdown", "HwThermalSlowdown", "SwThermalSlowdown"}
+        reasons = sorted(r for r in self.reasons if r not in ("None", "GpuIdle", "All", "ApplicationsClocksSetting"))
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": reasons, "samples": len(self.samples),
+                "rejected": bool(bad & set(reasons))}
+
+
+def oracle_sample(w, target_points=3_000_000):
+    """Bounded sample of the workload for the CPU oracle: the active points of a slab ix in [lo, hi) of the
+    same box and potential (a truncated shell; psi = 0 outside it), about `target_points` points."""
+    from oracle import gpe_oracle as O
+    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center)
+    pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
+    plane = w.ny * w.nz
+    mid = w.nx // 2
+    parts, total, lo, hi = [], 0, mid, mid
+    # grow a slab outwards from the centre plane until it holds enough points
+    while total < target_points and (lo > 0 or hi < w.nx):
+        for ix in ([hi] if hi < w.nx else []) + ([lo - 1] if lo > 0 else []):
+            v = O.mask_potential_plane(box, pot, w.mask_mode, ix)
+            idx = np.nonzero((v < w.v_cut).ravel())[0].astype(np.int64) + ix * plane
+            parts.append(idx)
+            total += idx.size
+        hi = min(hi + 1, w.nx)
+        lo = max(lo - 1, 0)
+    act = np.sort(np.concatenate(parts)) if parts else np.zeros(0, np.int64)
+    return box, pot, act, f"active points with {lo} <= ix < {hi} of {w.name} ({act.size} of the shell's points)"
+
+
+def time_oracle(w, steps, warmup=1, target_points=3_000_000):
+    """RK4 steps of the C oracle (textbook k1..k4, explicit loops, OpenMP over the host cores) on the sample."""
+    from oracle import c_oracle as CO
+    box, pot, act, what = oracle_sample(w, target_points)
+    co = CO.COracle(box, pot, act, w.stencil)
+    psi = I.make_psi0(w, act)
+    for _ in range(warmup):
+        psi = co.run_rk4(w.g, 0.0, w.dt, 1, psi)
+    t0 = time.perf_counter()
+    psi = co.run_rk4(w.g, warmup * w.dt, w.dt, steps, psi)
+    el = time.perf_counter() - t0
+    assert np.all(np.isfinite(psi))
+    return {"value": act.size * 4 * steps / el, "unit": UNIT, "cores": co.threads, "kind": "oracle",
+            "sample": f"{steps} RK4 steps on the {what}", "seconds": el}, act.size, el
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    base, n, _ = time_oracle(w, 1, warmup=0, target_points=1_500_000)   # size the sample
+    per_step = base["seconds"]
+    tp = 1_500_000 if per_step * (args.steps + args.warmup) < 200 else 400_000
+    res, n, el = time_oracle(w, args.steps, warmup=args.warmup, target_points=tp)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
+        "config": {"workload": w.name, "stencil": w.stencil, "sample": res["sample"]},
+        "cpu_baseline": {k: res[k] for k in ("value", "unit", "cores", "kind", "sample")},
+        "e2e": {"value": res["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+    import paper_2603_05447_b200 as P
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the GPE path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- a1: layout build (host), once per grid ------------------------------------------------
+    t0 = time.perf_counter()
+    grid = P.Grid.from_workload(w)
+    t_layout = time.perf_counter() - t0
+    n = grid.n_active
+    info = grid.layout_info()
+    sim = P.Sim(grid, w.dtype, w.stencil, w.g, device=f"cuda:{local}")
+    if args.kz:
+        sim.set_planes_per_block(args.kz)
+    csize = 16 if w.dtype == "complex128" else 8
+    act = grid.active_indices()
+    psi0 = I.make_psi0(w, act).astype(sim.npdtype)
+    host = torch.empty(n, dtype=sim.cdtype).pin_memory()
+    host_np = host.numpy()
+    host_np[:] = psi0
+    sim.set_psi_host(host_np)
+    sim.time = 0.0
+    stream = torch.cuda.current_stream()
+
+    # ---- device-resident timing: W warm-up steps, K timed steps ------------------------------------
+    sampler = ClockSampler(local)
+    for _ in range(args.warmup):
+        sim.run_rk4(w.dt, 1)
+    barrier()
+    sampler.start()
+    sim.time_stages(True)
+    l0 = sim.kernel_launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        sim.run_rk4(w.dt, 1)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    stage_ms, stage_cnt = sim.stage_time_ms()
+    sim.time_stages(False)
+    launches = sim.kernel_launches - l0
+    if world > 1:
+        tmax = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms = float(tmax.item())
+        ntot = torch.tensor([n], device=dev, dtype=torch.float64)
+        dist.all_reduce(ntot, op=dist.ReduceOp.SUM)
+        n_all = float(ntot.item())
+    else:
+        n_all = float(n)
+    value = n_all * 4 * args.steps / (ms * 1e-3)
+    nrm = sim.norm()
+    if not (abs(nrm - 1.0) < 1e-2):
+        raise SystemExit(f"bench.py: state lost normalisation ({nrm}); the run is invalid")
+
+    # ---- roofline of the dominant stage kernel (live CUDA-event durations of every stage launch) -----
+    peak, peak_src = measured_peak()
+    stages = []
+    for k in range(4):
+        if stage_cnt[k]:
+            avg_ms = stage_ms[k] / stage_cnt[k]
+            by = STAGE_ELEMS[k] * csize * n
+            stages.append({"kernel": f"stage_kernel<S{k + 1}>", "avg_ms": avg_ms, "algorithmic_bytes": by,
+                           "GBps": by / (avg_ms * 1e-3) / 1e9, "frac": by / (avg_ms * 1e-3) / 1e9 / peak})
+    dom = max(stages, key=lambda s: s["avg_ms"]) if stages else None
+    tot_ms = sum(s["avg_ms"] for s in stages)
+    tot_by = sum(s["algorithmic_bytes"] for s in stages)
+    roofline = None
+    if dom:
+        dkey = "c128" if w.dtype == "complex128" else "c64"
+        roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["GBps"], "peak": peak, "unit": "GB/s",
+                    "frac": dom["frac"], "traffic": recorded_traffic(w.name, dkey), "peak_source": peak_src,
+                    "frac_of_8TBps": dom["GBps"] / 8000.0,
+                    "all_stages": {"achieved": tot_by / (tot_ms * 1e-3) / 1e9, "frac": tot_by / (tot_ms * 1e-3) / 1e9 / peak,
+                                   "stage_share_of_step": tot_ms * args.steps / ms if world == 1 else None},
+                    "stages": stages}
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D psi, one RK4 step, D2H psi ------
+    e2e_steps = max(1, min(args.steps, 3))
+    out_host = torch.empty(n, dtype=sim.cdtype).pin_memory()
+    out_np = out_host.numpy()
+    sim.set_psi_host(host_np)
+    sim.run_rk4(w.dt, 1)
+    sim.get_psi_host(out_np)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sim.set_psi_host(host_np)
+        sim.run_rk4(w.dt, 1)
+        sim.get_psi_host(out_np)
+    torch.cuda.synchronize(dev)
+    t_e2e = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_e2e = float(tt.item())
+    e2e = {"value": n_all * 4 * e2e_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": n * csize,
+           "d2h_bytes_per_step": n * csize, "steps": e2e_steps,
+           "call": "gpe_set_psi_host + gpe_run_rk4(1) + gpe_get_psi_host per step, pinned host buffers"}
+
+    # ---- the other rows of the path, timed outside the headline region --------------------------------
+    def timed(fn, reps):
+        fn()
+        torch.cuda.synchronize(dev)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(reps):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize(dev)
+        return a.elapsed_time(b) / reps
+
+    sim.set_psi_host(host_np)
+    extra = {"layout_build_s": t_layout, "n_tiles": info.n_tiles, "n_work_items": info.n_work}
+    ms_imag = timed(lambda: sim.run_imag(w.dt, 10), 2) / 10
+    extra["imag_step"] = {"ms": ms_imag, "point_updates_per_s": n / (ms_imag * 1e-3), "GBps": 2 * csize * n / (ms_imag * 1e-3) / 1e9}
+    ms_en = timed(lambda: sim.energy(), 3)
+    extra["energy"] = {"ms": ms_en, "GBps": csize * n / (ms_en * 1e-3) / 1e9}
+    ms_nm = timed(lambda: sim.norm(), 3)
+    extra["norm"] = {"ms": ms_nm, "GBps": csize * n / (ms_nm * 1e-3) / 1e9}
+    d = sim.get_psi()
+    ms_pk = timed(lambda: sim.set_psi(d), 3)
+    extra["pack"] = {"ms": ms_pk}
+
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample -------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        res, _, _ = time_oracle(w, 2, warmup=1, target_points=3_000_000)
+        cpu = {k: res[k] for k in ("value", "unit", "cores", "kind", "sample")}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "c128" if w.dtype == "complex128" else "c64", "data": "synthetic",
+        "config": {"workload": w.name, "box": [w.nx, w.ny, w.nz], "h": w.h, "stencil": w.stencil, "n_active": n,
+                   "active_fraction": n / (w.nx * w.ny * w.nz), "dt": w.dt, "g": w.g,
+                   "planes_per_block": args.kz or "default", "parallelism": "replicas" if world > 1 else "single",
+                   "l2": "inputs larger than L2 (no flush)" if n * csize > 2 * 126e6 else "inputs fit L2: flushless, L2-resident"},
+        "hbm_GBps_algorithmic": value * 3 * csize / 1e9 / world,
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+        "extra": extra,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4_c128", choices=sorted(workloads()))
+    ap.add_argument("--kz", type=int, default=0, help="planes per thread block (0 = library default)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = workloads()[args.workload]
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

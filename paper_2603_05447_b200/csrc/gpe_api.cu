@@ -29,7 +29,7 @@ struct gpe_sim {
     int radius = 1;
     double g = 0.0, n_target = 1.0;
     double t = 0.0;
-    int kz = 16;
+    int kz = 32;
     size_t csize = 16;      // bytes per complex value
     int64_t n = 0;          // n_active
     void* buf[4] = {nullptr, nullptr, nullptr, nullptr};  // A (psi), B, C, D in storage order
@@ -173,6 +173,18 @@ StageParams base_params(const gpe_sim* s, double t) {
     p.g = s->g;
     p.partials = s->d_partials;
     p.scale_in = s->d_sums + NACC;
+    const GridHost& h = s->grid->h;
+    const double ih2 = -0.5 / (h.box.h * h.box.h);
+    p.kw[0] = ih2 * 3.0 * (s->radius == 1 ? -2.0 : -2.5);
+    p.kw[1] = ih2 * (s->radius == 1 ? 1.0 : 4.0 / 3.0);
+    p.kw[2] = s->radius == 1 ? 0.0 : ih2 * (-1.0 / 12.0);
+    for (int k = 0; k < 3; ++k) p.kwf[k] = (float)p.kw[k];
+    p.xc = 0.5 * (double)(h.box.nx - 1);
+    p.yc = 0.5 * (double)(h.box.ny - 1);
+    p.zc = 0.5 * (double)(h.box.nz - 1);
+    p.hax = 0.5 * h.pot.ax; p.hay = 0.5 * h.pot.ay; p.haz = 0.5 * h.pot.az;
+    p.om2 = h.pot.omega * h.pot.omega;
+    p.delta_eff = h.pot.kind == GPE_POT_DRESSED ? p.pot.delta : 0.0;
     return p;
 }
 
@@ -333,6 +345,7 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     const int radius = stencil == 7 ? 1 : 2;
     if (g->h.tx != 8 || g->h.ty != 8) return fail(GPE_ERR_UNSUPPORTED, "kernels need 8x8 column tiles");
     if (g->h.halo_width < radius) return fail(GPE_ERR_UNSUPPORTED, "grid halo_width is smaller than the stencil radius");
+    if (g->h.n_active >= ((int64_t)1 << 32)) return fail(GPE_ERR_UNSUPPORTED, "more than 2^32-1 active points (kernels index storage with 32 bits)");
     if (((uintptr_t)dev_state & 255) != 0) return fail(GPE_ERR_INVALID_ARG, "dev_state must be 256-byte aligned");
     const size_t bb = buf_bytes(g->h.n_active, dtype);
     if (state_bytes < 5 * bb) return fail(GPE_ERR_INVALID_ARG, "state_bytes too small (see gpe_sim_state_bytes)");
@@ -347,7 +360,7 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     s->n_target = n_target;
     s->csize = dtype == GPE_C128 ? 16 : 8;
     s->n = g->h.n_active;
-    s->kz = 16;
+    s->kz = 32;
     for (int k = 0; k < 4; ++k) s->buf[k] = (char*)dev_state + k * bb;
     s->staging = (char*)dev_state + 4 * bb;
     cudaError_t e = cudaMalloc(&s->d_sums, (NACC + 1) * sizeof(double));
@@ -548,8 +561,7 @@ int gpe_sim_stage_time_ms(gpe_sim* s, double ms_out[4], int64_t count_out[4]) {
 
 int gpe_sim_set_planes_per_block(gpe_sim* s, int kz) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
-    if (kz < 1 || kz > 32) return fail(GPE_ERR_INVALID_ARG, "planes per block must be in 1..32");
-    if (stage_smem_bytes(s->dtype, s->radius, kz) > 200 * 1024) return fail(GPE_ERR_INVALID_ARG, "tile does not fit shared memory");
+    if (kz < 1 || kz > 4096) return fail(GPE_ERR_INVALID_ARG, "planes per stream must be in 1..4096");
     CU(cudaDeviceSynchronize());
     s->kz = kz;
     return build_work(s);

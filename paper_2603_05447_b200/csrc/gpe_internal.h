@@ -58,7 +58,7 @@ struct Slab {                // one z-plane of one tile
     long long base;          // storage position of the slab's first lane
 };
 
-// One thread block's worth of work: nz consecutive planes of one tile (a piece of a work item).
+// One stream (half-warp's worth of work): nz consecutive planes of one tile (a piece of a work item).
 // eoff[q] + zp = slab entry of plane zp in tile q (0 = own, 1..4 = -x,+x,-y,+y), valid for
 // zlo[q] <= zp < zhi[q] (zlo = zhi = 0 when the neighbour tile is absent).
 struct alignas(16) WorkRec {
@@ -92,16 +92,24 @@ enum Mode : int {
     MODE_ENERGY = 6  // partial sums of Re(conj(c) T c), V|c|^2, |c|^4, |c|^2
 };
 constexpr int NACC = 4;           // accumulators per block in the partial-sum array
-constexpr int STAGE_THREADS = 256;
+constexpr int STAGE_THREADS = 128;
 
 struct StageParams {
     const Slab* slabs;
     const WorkRec* work;
     int32_t n_work;
-    int32_t kz;            // max planes per block (smem tile is sized for it)
+    int32_t kz;            // max planes per stream (informational; the split is done on the host)
     PotDev pot;
     double g;
     double ca;             // stage coefficient (dt/2, dt, dt/6, or dt of the imaginary step)
+    // host-precomputed constants (read from the parameter bank, no registers):
+    double kw[3];          // -1/(2h^2) * {3 c_0, c_1, c_2} of the stencil
+    float kwf[3];          // the same in fp32 (complex64 state)
+    float padf;
+    double xc, yc, zc;     // 0.5 (n-1) per axis: coordinate = (i - xc) h + cx
+    double hax, hay, haz;  // 0.5 a_x, 0.5 a_y, 0.5 a_z
+    double om2;            // Omega^2
+    double delta_eff;      // Delta(t) for the dressed potential, 0 for the harmonic one
     const void* in;        // array the stencil is applied to (storage order)
     const void* aux;       // y0 or p (storage order) or null
     void* out1;
@@ -112,7 +120,7 @@ struct StageParams {
 
 // Launchers (gpe_kernels.cu).  dtype: GPE_C64 / GPE_C128; radius 1 or 2.  Return cudaError_t as int.
 int launch_stage(int dtype, int radius, int mode, const StageParams& p, void* stream);
-size_t stage_smem_bytes(int dtype, int radius, int kz);
+size_t stage_smem_bytes(int dtype, int radius);
 int launch_pack(int dtype, const void* canonical, void* storage, const int64_t* perm, int64_t n, void* stream);
 int launch_unpack(int dtype, const void* storage, void* canonical, const int64_t* perm, int64_t n, void* stream);
 // partials[b*NACC + 0] = sum over the block's contiguous chunk of |psi|^2; nblk = norm_blocks(n)

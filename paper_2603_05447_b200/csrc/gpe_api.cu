@@ -561,7 +561,7 @@ int gpe_sim_stage_time_ms(gpe_sim* s, double ms_out[4], int64_t count_out[4]) {
 
 int gpe_sim_set_planes_per_block(gpe_sim* s, int kz) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
-    if (kz < 1 || kz > 4096) return fail(GPE_ERR_INVALID_ARG, "planes per stream must be in 1..4096");
+    if (kz < 1 || kz > stage_max_planes()) return fail(GPE_ERR_INVALID_ARG, "planes per stream must be in 1..32");
     CU(cudaDeviceSynchronize());
     s->kz = kz;
     return build_work(s);

@@ -121,6 +121,7 @@ struct StageParams {
 // Launchers (gpe_kernels.cu).  dtype: GPE_C64 / GPE_C128; radius 1 or 2.  Return cudaError_t as int.
 int launch_stage(int dtype, int radius, int mode, const StageParams& p, void* stream);
 size_t stage_smem_bytes(int dtype, int radius);
+int stage_max_planes();   // upper bound of WorkRec::nz the stage kernels accept
 int launch_pack(int dtype, const void* canonical, void* storage, const int64_t* perm, int64_t n, void* stream);
 int launch_unpack(int dtype, const void* storage, void* canonical, const int64_t* perm, int64_t n, void* stream);
 // partials[b*NACC + 0] = sum over the block's contiguous chunk of |psi|^2; nblk = norm_blocks(n)

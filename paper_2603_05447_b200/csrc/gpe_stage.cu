@@ -1,0 +1,532 @@
+// Fused stage kernels (sm_100a) of the sparse-grid Gross-Pitaevskii hot path: stencil + V(r,t) + nonlinear
+// term + Runge-Kutta / imaginary-time combination over the 8x8-column-tile layout, one launch per stage.
+//
+//   H[psi;t] psi = -1/2 lap_h psi + V(r,t) psi + g|psi|^2 psi      PAPER.md:27 Eq. 2, :71 Eq. 8
+//   psi = 0 outside the region of interest
+//   RK4 in stage-state form                                        PAPER.md:276-281 Eq. A6-A7, :315-319 A10-A11
+//   imaginary time: Euler step + particle-number partial sums,
+//   renormalisation applied lazily at the next load                PAPER.md:60 Eq. 6, :87 (kernels K1-K3)
+//
+// Work decomposition: a STREAM is one WorkRec = nz <= 32 consecutive z-planes of one
+// 8x8 column tile.  A half-warp (16 lanes) marches one stream along z.  Lane t = (g, ly) = (t / 8, t % 8)
+// owns the 4x1 patch rows lx = 4g .. 4g+3 of column ly of every plane, so
+//   - for a fixed patch element the 8 lanes of a row touch CONSECUTIVE storage positions: every global
+//     load / store and every shared-memory access of the half-warp is a run of contiguous 16-byte values
+//     (full 32-byte sectors, no bank conflicts),
+//   - z neighbours never leave registers (accumulate-forward form: psi(k-1..k-R) and the partial sums of
+//     T psi for planes k-1..k-R are the only state),
+//   - the x neighbours inside the patch are the lane's own registers.
+// Tables: the slab entries (64-bit mask + storage base) of the own tile and of the four neighbour tiles for
+// the planes the stream touches are copied to shared memory once at stream start; no table load sits on the
+// per-plane critical path.
+// Per plane: cp.async (zero-filled where the mask bit is clear: Dirichlet psi = 0) of the own patch, of the
+// lane's share of the star halo (edge rows / columns of the four neighbour tiles) and of the aux operand
+// (y0 or p) into rings of plane slots, PF planes in flight; one __syncwarp per plane, no block-level barrier.
+// Plane c = k-R is finished when plane k has arrived: V(r,t) analytic, nonlinear term, stage combination,
+// row-contiguous stores.  IMAG / ENERGY: per-stream partial sums in a fixed order -> partials[stream].
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "gpe_internal.h"
+
+namespace gpe {
+
+namespace {
+
+template <typename T> struct CxOf;
+template <> struct CxOf<double> { using type = double2; };
+template <> struct CxOf<float> { using type = float2; };
+
+template <typename T> __device__ __forceinline__ typename CxOf<T>::type mk(T a, T b);
+template <> __device__ __forceinline__ double2 mk<double>(double a, double b) { return make_double2(a, b); }
+template <> __device__ __forceinline__ float2 mk<float>(float a, float b) { return make_float2(a, b); }
+
+// cp.async of one complex value with zero fill (src-size 0 reads nothing and writes zeros: Dirichlet psi = 0)
+__device__ __forceinline__ void cp_async_zfill(unsigned smem_dst, const double2* src, bool valid) {
+    const int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_dst), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_zfill(unsigned smem_dst, const float2* src, bool valid) {
+    const int sz = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_dst), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ double2 lds_c(unsigned addr, double2*) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float2 lds_c(unsigned addr, float2*) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint2 lds_u2(unsigned addr) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];\n" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ unsigned lds_u1(unsigned addr) {
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];\n" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts_u2(unsigned addr, unsigned a, unsigned b) {
+    asm volatile("st.shared.v2.u32 [%0], {%1, %2};\n" ::"r"(addr), "r"(a), "r"(b) : "memory");
+}
+__device__ __forceinline__ void sts_u1(unsigned addr, unsigned a) {
+    asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(addr), "r"(a) : "memory");
+}
+
+// sqrt(s) for s >= 0 from the hardware reciprocal-square-root seed and two coupled Newton steps
+// (relative error a few 1e-16; the IEEE-rounded sqrt() costs about twice the FP64 instructions).
+__device__ __forceinline__ double fast_sqrt(double s) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;\n" : "=d"(y) : "d"(s));
+    double g = s * y, h = 0.5 * y;
+    double r = fma(-g, h, 0.5);
+    g = fma(g, r, g);
+    h = fma(h, r, h);
+    r = fma(-g, h, 0.5);
+    g = fma(g, r, g);
+    h = fma(h, r, h);
+    r = fma(-g, g, s);          // residual s - g^2
+    g = fma(r, h, g);
+    return s > 0.0 ? g : 0.0;
+}
+
+constexpr int KZMAX = 32;                 // planes per stream (host splits work items to at most this)
+constexpr int PF = 2;                     // planes in flight per stream (cp.async groups)
+constexpr int NSLOT = PF + 1;             // ring of plane slots per stream
+constexpr int NAUX = PF + 1;              // ring of aux-plane slots per stream
+constexpr int STAGE_WARPS = STAGE_THREADS / 32;
+constexpr int STREAMS_PER_BLOCK = 2 * STAGE_WARPS;
+
+// Shared memory of one stream.  Plane slot: (8+2R) rows (x) of PY values, the tile at rows/cols R..R+7 and
+// the star halo around it.  For 8-byte values and R = 2 the pitch is 14 so that the two row groups of a
+// half-warp (4 rows apart) fall into different banks.
+template <typename T, int R, bool AUX> struct Geo {
+    static constexpr int ES = 2 * (int)sizeof(T);
+    static constexpr int ROWS = 8 + 2 * R;
+    static constexpr int PY = (sizeof(T) == 4 && R == 2) ? 14 : 8 + 2 * R;
+    static constexpr int PLANE = ROWS * PY;                 // values per slot
+    static constexpr int NE = KZMAX + 2 * R;                // table entries per tile
+    static constexpr int RING_BYTES = NSLOT * PLANE * ES;
+    static constexpr int AUX_BYTES = AUX ? NAUX * 64 * ES : 0;
+    static constexpr int MASK_OFF = RING_BYTES + AUX_BYTES;  // [5][NE] (lo, hi)
+    static constexpr int BASE_OFF = MASK_OFF + 5 * NE * 8;   // [5][NE] storage base
+    static constexpr int STREAM_BYTES = (BASE_OFF + 5 * NE * 4 + 15) / 16 * 16;
+    __host__ __device__ static constexpr int at(int r, int c) { return (r + R) * PY + (c + R); }
+};
+
+template <typename T> struct KW;   // stencil weights of the right type straight from the parameter block
+template <> struct KW<double> {
+    static __device__ __forceinline__ double w(const StageParams& p, int s) { return p.kw[s]; }
+};
+template <> struct KW<float> {
+    static __device__ __forceinline__ float w(const StageParams& p, int s) { return p.kwf[s]; }
+};
+
+__host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
+
+template <typename T, int R, int MODE>
+__global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage_kernel(const __grid_constant__ StageParams p) {
+    using C = typename CxOf<T>::type;
+    constexpr bool HAS_AUX = mode_has_aux(MODE);
+    using G = Geo<T, R, HAS_AUX>;
+    constexpr unsigned ES = G::ES;
+    constexpr int NHE = 2 * R;                             // halo values per lane and plane
+    constexpr unsigned SLOT_BYTES = (unsigned)G::PLANE * ES;
+    constexpr unsigned ROW_BYTES = (unsigned)G::PY * ES;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int half = lane >> 4, t = lane & 15;
+    const int g = t >> 3, ly = t & 7;                      // row group and column of the 4x1 patch
+    const int sidx = (blockIdx.x * STAGE_WARPS + warp) * 2 + half;   // this half-warp's stream
+    const bool valid = sidx < p.n_work;
+    const WorkRec* __restrict__ w = p.work + (valid ? sidx : 0);
+
+    const int z0 = w->z0, nz = valid ? w->nz : 0;
+    const int kstart = z0 - R;
+    const int ne = nz > 0 ? nz + 2 * R : 0;                // planes kstart .. kstart+ne-1 are touched
+
+    const unsigned sb = (unsigned)__cvta_generic_to_shared(smem_raw) + (unsigned)((warp * 2 + half) * G::STREAM_BYTES);
+    const unsigned ring = sb, auxring = sb + G::RING_BYTES, smask = sb + G::MASK_OFF, sbase = sb + G::BASE_OFF;
+
+    // ---- slab tables of the five tiles -> shared memory (all loads in flight at once) ----------------
+    {
+        constexpr int NM = (G::NE + 15) / 16;
+        unsigned tl[5 * NM], th[5 * NM], tb[5 * NM];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+            const int zl = w->zlo[q], zh = w->zhi[q];
+            const Slab* __restrict__ tab = p.slabs + w->eoff[q];
+#pragma unroll
+            for (int m = 0; m < NM; ++m) {
+                const int i = t + 16 * m, zp = kstart + i;
+                tl[q * NM + m] = 0u; th[q * NM + m] = 0u; tb[q * NM + m] = 0u;
+                if (i < ne && zp >= zl && zp < zh) {
+                    const uint4 s = __ldg(reinterpret_cast<const uint4*>(tab + zp));
+                    tl[q * NM + m] = s.x; th[q * NM + m] = s.y; tb[q * NM + m] = s.z;
+                }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+#pragma unroll
+            for (int m = 0; m < NM; ++m) {
+                const int i = t + 16 * m;
+                if (i < G::NE) {
+                    sts_u2(smask + (unsigned)((q * G::NE + i) * 8), tl[q * NM + m], th[q * NM + m]);
+                    sts_u1(sbase + (unsigned)((q * G::NE + i) * 4), tb[q * NM + m]);
+                }
+            }
+    }
+
+    // ---- lane constants ---------------------------------------------------------------------------------
+    unsigned bm[4];                                        // bits below own element e inside its word
+#pragma unroll
+    for (int e = 0; e < 4; ++e) bm[e] = (1u << (8 * e + ly)) - 1u;
+    const unsigned own_off = (unsigned)G::at(4 * g, ly) * ES;          // + e * ROW_BYTES
+    const unsigned aux_off = (unsigned)(32 * g + ly) * ES;             // + e * 8 * ES
+    // halo duty: neighbour tile hq (0..3 = -x,+x,-y,+y), values 4e + j of its 8R-value edge
+    const int hq = t >> 2, hj = t & 3;
+    unsigned hbm[NHE], hoff[NHE];
+#pragma unroll
+    for (int e = 0; e < NHE; ++e) {
+        const int idx = 4 * e + hj;
+        int nlx, nly, drow, dcol;
+        if (hq < 2) {
+            const int rr = idx >> 3, cc = idx & 7;
+            nlx = hq == 0 ? 8 - R + rr : rr; nly = cc;
+            drow = hq == 0 ? rr - R : 8 + rr; dcol = cc;
+        } else {
+            const int rr = idx / R, cc = idx % R;
+            nlx = rr; nly = hq == 2 ? 8 - R + cc : cc;
+            drow = rr; dcol = hq == 2 ? cc - R : 8 + cc;
+        }
+        hbm[e] = (1u << ((nlx * 8 + nly) & 31)) - 1u;
+        hoff[e] = (unsigned)((drow + R) * G::PY + (dcol + R)) * ES;
+    }
+    const bool selA = hq == 0, selB = hq != 1;             // word (hi?) of values e < NHE/2 and e >= NHE/2
+
+    const C* __restrict__ in = reinterpret_cast<const C*>(p.in);
+    const C* __restrict__ auxp = reinterpret_cast<const C*>(p.aux);
+
+    // potential: u = qxy[e] + qz(plane); qxy = 1/2 (ax x^2 + ay y^2) of the patch points
+    double qxy[4];
+    {
+        const double y = ((double)(w->iy0 + ly) - p.yc) * p.pot.h + p.pot.cy;
+        const double qy = p.hay * (y * y);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const double x = ((double)(w->ix0 + 4 * g + e) - p.xc) * p.pot.h + p.pot.cx;
+            qxy[e] = fma(p.hax, x * x, qy);
+        }
+    }
+    double sc = 1.0, gsc = p.g;
+    if (MODE == MODE_IMAG) { sc = *p.scale_in; gsc = p.g * (sc * sc); }
+
+    int niter = ne;
+    niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16));   // both halves run the same loop
+    __syncwarp();                                                  // tables visible to the half-warp
+
+    // ---- producer: plane index i (plane kstart + i) -> slot sp; aux of plane i - R -> aux slot ap ------
+    auto produce = [&](const int i, const unsigned sp, const unsigned ap) {
+        if (i < ne) {
+            {
+                const uint2 m = lds_u2(smask + (unsigned)i * 8u);
+                const unsigned word = g ? m.y : m.x;
+                const unsigned bc = lds_u1(sbase + (unsigned)i * 4u) + (g ? (unsigned)__popc(m.x) : 0u);
+                const unsigned dst = ring + sp * SLOT_BYTES + own_off;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const bool on = (word >> (8 * e + ly)) & 1u;
+                    cp_async_zfill(dst + (unsigned)e * ROW_BYTES, in + (bc + (unsigned)__popc(word & bm[e])), on);
+                }
+            }
+            if (i >= R && i < ne - R) {
+                const unsigned ti = (unsigned)((1 + hq) * G::NE + i);
+                const uint2 m = lds_u2(smask + ti * 8u);
+                const unsigned b = lds_u1(sbase + ti * 4u);
+                const unsigned pl = (unsigned)__popc(m.x);
+                const unsigned wA = selA ? m.y : m.x, wB = selB ? m.y : m.x;
+                const unsigned bA = b + (selA ? pl : 0u), bB = b + (selB ? pl : 0u);
+                const unsigned dst = ring + sp * SLOT_BYTES;
+#pragma unroll
+                for (int e = 0; e < NHE; ++e) {
+                    const unsigned ww = e < NHE / 2 ? wA : wB, bb = e < NHE / 2 ? bA : bB;
+                    const bool on = (ww & (hbm[e] + 1u)) != 0u;
+                    cp_async_zfill(dst + hoff[e], in + (bb + (unsigned)__popc(ww & hbm[e])), on);
+                }
+            }
+            if (HAS_AUX) {
+                const int ia = i - R;
+                if (ia >= R && ia < ne - R) {
+                    const uint2 m = lds_u2(smask + (unsigned)ia * 8u);
+                    const unsigned word = g ? m.y : m.x;
+                    const unsigned bc = lds_u1(sbase + (unsigned)ia * 4u) + (g ? (unsigned)__popc(m.x) : 0u);
+                    const unsigned dst = auxring + ap * (64u * ES) + aux_off;
+#pragma unroll
+                    for (int e = 0; e < 4; ++e)
+                        if ((word >> (8 * e + ly)) & 1u)
+                            cp_async_zfill(dst + (unsigned)e * (8u * ES), auxp + (bc + (unsigned)__popc(word & bm[e])), true);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+
+    // state (accumulate-forward form): set s holds psi and the partial T psi of one earlier plane
+    C SP[R][4], SA[R][4];
+#pragma unroll
+    for (int s = 0; s < R; ++s)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { SP[s][e] = mk<T>((T)0, (T)0); SA[s][e] = mk<T>((T)0, (T)0); }
+    double acc[NACC] = {0.0, 0.0, 0.0, 0.0};
+
+    // ---- prologue: planes 0 .. PF-1 in flight ----------------------------------------------------------------
+#pragma unroll
+    for (int i = 0; i < PF; ++i) produce(i, (unsigned)i, (unsigned)((i + NAUX - (R % NAUX)) % NAUX));
+
+    // one plane step at plane index i (plane k = kstart + i).  (PN, AN) = set of plane k-1, (PO, AO) = set of
+    // plane k-R (the same set for R = 1).  sl = ring slot of plane i; al = aux slot of plane i - R.
+    auto step = [&](C (&PN)[4], C (&AN)[4], C (&PO)[4], C (&AO)[4], const int i, const unsigned sl, const unsigned al) {
+        cp_async_wait<PF - 1>();
+        __syncwarp();
+        {
+            unsigned sp = sl + PF, ap = al + PF;
+            if (sp >= NSLOT) sp -= NSLOT;
+            if (ap >= NAUX) ap -= NAUX;
+            produce(i + PF, sp, ap);
+        }
+        if (i >= ne) return;
+        const unsigned so = ring + sl * SLOT_BYTES + own_off;   // own patch in the slot of plane k
+        const int ic = i - R;                                   // plane finished in this step
+        // ---- output plane: activity bits and storage positions --------------------------------------------
+        unsigned cword = 0u, cbase = 0u;
+        if (ic >= R) {
+            const uint2 m = lds_u2(smask + (unsigned)ic * 8u);
+            cword = g ? m.y : m.x;
+            cbase = lds_u1(sbase + (unsigned)ic * 4u) + (g ? (unsigned)__popc(m.x) : 0u);
+        }
+        // ---- psi(k) of the patch ------------------------------------------------------------------------
+        C v[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) v[e] = lds_c(so + (unsigned)e * ROW_BYTES, (C*)nullptr);
+        // ---- psi(k) completes the z part of planes k-1 .. k-R -------------------------------------------
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            AO[e].x = fma(KW<T>::w(p, R), v[e].x, AO[e].x);
+            AO[e].y = fma(KW<T>::w(p, R), v[e].y, AO[e].y);
+            if (R == 2) {
+                AN[e].x = fma(KW<T>::w(p, 1), v[e].x, AN[e].x);
+                AN[e].y = fma(KW<T>::w(p, 1), v[e].y, AN[e].y);
+            }
+        }
+        // ---- finish plane c = k - R: V(r,t), nonlinear term, stage combination --------------------------------
+        if (cword) {
+            const double zc = ((double)(kstart + ic) - p.zc) * p.pot.h + p.pot.cz;
+            const double qz = p.haz * (zc * zc) - p.delta_eff;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const bool on = (cword >> (8 * e + ly)) & 1u;
+                const unsigned pos = cbase + (unsigned)__popc(cword & bm[e]);
+                const C cv = PO[e];
+                const C tc = AO[e];
+                C av = mk<T>((T)0, (T)0);
+                if (HAS_AUX) av = lds_c(auxring + al * (64u * ES) + aux_off + (unsigned)e * (8u * ES), (C*)nullptr);
+                double vpot = qxy[e] + qz;
+                if (p.pot.kind == GPE_POT_DRESSED) vpot = fast_sqrt(fma(vpot, vpot, p.om2)) - p.pot.omega;
+                const T a2 = fma(cv.x, cv.x, cv.y * cv.y);
+                if (MODE == MODE_ENERGY) {
+                    if (on) {
+                        acc[0] += (double)(cv.x * tc.x + cv.y * tc.y);
+                        acc[1] += vpot * (double)a2;
+                        acc[2] += (double)a2 * (double)a2;
+                        acc[3] += (double)a2;
+                    }
+                    continue;
+                }
+                const T diag = (T)fma(gsc, (double)a2, vpot);
+                const C hc = mk<T>(fma(diag, cv.x, tc.x), fma(diag, cv.y, tc.y));
+                const T ca = (T)p.ca;
+                C o;
+                if (MODE == MODE_APPLY) {
+                    o = hc;
+                } else if (MODE == MODE_IMAG) {
+                    const T s = (T)sc;
+                    o = mk<T>(s * fma(-ca, hc.x, cv.x), s * fma(-ca, hc.y, cv.y));
+                    if (on) acc[0] += (double)o.x * (double)o.x + (double)o.y * (double)o.y;
+                } else {
+                    // f = -i H c = (hc.y, -hc.x)
+                    const C base = (MODE == MODE_S1) ? cv : av;
+                    o = mk<T>(fma(ca, hc.y, base.x), fma(-ca, hc.x, base.y));
+                    if (MODE == MODE_S4) {
+                        const T third = (T)(1.0 / 3.0);
+                        o.x = fma(third, cv.x, o.x);
+                        o.y = fma(third, cv.y, o.y);
+                    }
+                    if (MODE == MODE_S2) {
+                        const T third = (T)(1.0 / 3.0), tt = (T)(2.0 / 3.0);
+                        if (on)
+                            reinterpret_cast<C*>(p.out2)[pos] =
+                                mk<T>(fma(tt, o.x, third * (cv.x - av.x)), fma(tt, o.y, third * (cv.y - av.y)));
+                    }
+                }
+                if (on) reinterpret_cast<C*>(p.out1)[pos] = o;
+            }
+        }
+        // ---- the oldest set becomes the set of plane k: z-backward part, centre ---------------------------------
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            C an;
+            if (R == 2) {
+                an.x = KW<T>::w(p, 2) * PO[e].x;
+                an.y = KW<T>::w(p, 2) * PO[e].y;
+                an.x = fma(KW<T>::w(p, 1), PN[e].x, an.x);
+                an.y = fma(KW<T>::w(p, 1), PN[e].y, an.y);
+            } else {
+                an.x = KW<T>::w(p, 1) * PO[e].x;
+                an.y = KW<T>::w(p, 1) * PO[e].y;
+            }
+            AO[e].x = fma(KW<T>::w(p, 0), v[e].x, an.x);
+            AO[e].y = fma(KW<T>::w(p, 0), v[e].y, an.y);
+            PO[e] = v[e];
+        }
+        // ---- in-plane part (only planes of the stream itself are ever finished) ----------------------------------
+        if (i >= R && i < ne - R) {
+            // x direction: source rows r = -R .. 3+R of column ly; rows 0..3 are the patch itself
+#pragma unroll
+            for (int r = -R; r <= 3 + R; ++r) {
+                const C val = (r >= 0 && r <= 3) ? v[r] : lds_c(so + (unsigned)(r * (int)ROW_BYTES), (C*)nullptr);
+#pragma unroll
+                for (int a = 0; a < 4; ++a) {
+                    const int d = r > a ? r - a : a - r;
+                    if (d >= 1 && d <= R) {
+                        AO[a].x = fma(KW<T>::w(p, d), val.x, AO[a].x);
+                        AO[a].y = fma(KW<T>::w(p, d), val.y, AO[a].y);
+                    }
+                }
+            }
+            // y direction: columns ly +- 1 .. R of each patch row
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+#pragma unroll
+                for (int cc = -R; cc <= R; ++cc) {
+                    if (cc == 0) continue;
+                    const C val = lds_c(so + (unsigned)(a * (int)ROW_BYTES + cc * (int)ES), (C*)nullptr);
+                    const int d = cc > 0 ? cc : -cc;
+                    AO[a].x = fma(KW<T>::w(p, d), val.x, AO[a].x);
+                    AO[a].y = fma(KW<T>::w(p, d), val.y, AO[a].y);
+                }
+            }
+        }
+    };
+
+    unsigned sl = 0, al = (unsigned)((NAUX - (R % NAUX)) % NAUX);   // slots of plane index i and of plane i - R
+    for (int it = 0; it < niter; it += R) {
+        if (R == 1) {
+            step(SP[0], SA[0], SP[0], SA[0], it, sl, al);
+            sl = (sl + 1 == NSLOT) ? 0 : sl + 1;
+            al = (al + 1 == NAUX) ? 0 : al + 1;
+        } else {
+            step(SP[0], SA[0], SP[R - 1], SA[R - 1], it, sl, al);
+            sl = (sl + 1 == NSLOT) ? 0 : sl + 1;
+            al = (al + 1 == NAUX) ? 0 : al + 1;
+            if (it + 1 < niter) {
+                step(SP[R - 1], SA[R - 1], SP[0], SA[0], it + 1, sl, al);
+                sl = (sl + 1 == NSLOT) ? 0 : sl + 1;
+                al = (al + 1 == NAUX) ? 0 : al + 1;
+            }
+        }
+    }
+    cp_async_wait<0>();
+
+    // ---- per-stream partial sums in a fixed order (bit-reproducible, independent of scheduling) -------
+    if (MODE == MODE_IMAG || MODE == MODE_ENERGY) {
+#pragma unroll
+        for (int kq = 0; kq < NACC; ++kq)
+#pragma unroll
+            for (int off = 8; off > 0; off >>= 1) acc[kq] += __shfl_down_sync(0xffffffffu, acc[kq], off, 16);
+        if (t == 0 && valid) {
+#pragma unroll
+            for (int kq = 0; kq < NACC; ++kq) p.partials[(size_t)sidx * NACC + kq] = acc[kq];
+        }
+    }
+}
+
+template <typename T, int R, int MODE> constexpr size_t stage_smem() {
+    return (size_t)STREAMS_PER_BLOCK * Geo<T, R, mode_has_aux(MODE)>::STREAM_BYTES;
+}
+
+template <typename T, int R, int MODE>
+cudaError_t launch_one(const StageParams& p, cudaStream_t st) {
+    const int nblk = (p.n_work + STREAMS_PER_BLOCK - 1) / STREAMS_PER_BLOCK;
+    stage_kernel<T, R, MODE><<<nblk, STAGE_THREADS, stage_smem<T, R, MODE>(), st>>>(p);
+    return cudaGetLastError();
+}
+
+template <typename T, int R>
+cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
+    switch (mode) {
+        case MODE_APPLY: return launch_one<T, R, MODE_APPLY>(p, st);
+        case MODE_S1: return launch_one<T, R, MODE_S1>(p, st);
+        case MODE_S2: return launch_one<T, R, MODE_S2>(p, st);
+        case MODE_S3: return launch_one<T, R, MODE_S3>(p, st);
+        case MODE_S4: return launch_one<T, R, MODE_S4>(p, st);
+        case MODE_IMAG: return launch_one<T, R, MODE_IMAG>(p, st);
+        case MODE_ENERGY: return launch_one<T, R, MODE_ENERGY>(p, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <typename T, int R, int MODE>
+cudaError_t set_attr() {
+    return cudaFuncSetAttribute(stage_kernel<T, R, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)stage_smem<T, R, MODE>());
+}
+template <typename T, int R>
+cudaError_t set_attr_modes() {
+    cudaError_t e;
+    if ((e = set_attr<T, R, MODE_APPLY>())) return e;
+    if ((e = set_attr<T, R, MODE_S1>())) return e;
+    if ((e = set_attr<T, R, MODE_S2>())) return e;
+    if ((e = set_attr<T, R, MODE_S3>())) return e;
+    if ((e = set_attr<T, R, MODE_S4>())) return e;
+    if ((e = set_attr<T, R, MODE_IMAG>())) return e;
+    if ((e = set_attr<T, R, MODE_ENERGY>())) return e;
+    return cudaSuccess;
+}
+
+}  // namespace
+
+int stage_max_planes() { return KZMAX; }
+
+size_t stage_smem_bytes(int dtype, int radius) {   // largest over the modes (the aux-carrying RK stages)
+    if (dtype == GPE_C128) return radius == 1 ? stage_smem<double, 1, MODE_S2>() : stage_smem<double, 2, MODE_S2>();
+    return radius == 1 ? stage_smem<float, 1, MODE_S2>() : stage_smem<float, 2, MODE_S2>();
+}
+
+int kernels_configure() {
+    cudaError_t e;
+    if ((e = set_attr_modes<double, 1>())) return (int)e;
+    if ((e = set_attr_modes<double, 2>())) return (int)e;
+    if ((e = set_attr_modes<float, 1>())) return (int)e;
+    if ((e = set_attr_modes<float, 2>())) return (int)e;
+    return 0;
+}
+
+int launch_stage(int dtype, int radius, int mode, const StageParams& p, void* stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    if (p.n_work <= 0) return 0;
+    if (dtype == GPE_C128) return (int)(radius == 1 ? launch_mode<double, 1>(mode, p, st) : launch_mode<double, 2>(mode, p, st));
+    return (int)(radius == 1 ? launch_mode<float, 1>(mode, p, st) : launch_mode<float, 2>(mode, p, st));
+}
+
+}  // namespace gpe

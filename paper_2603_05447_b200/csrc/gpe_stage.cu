@@ -104,7 +104,6 @@ constexpr int PF = 2;                     // planes in flight per stream (cp.asy
 constexpr int NSLOT = PF + 1;             // ring of plane slots per stream
 constexpr int NAUX = PF + 1;              // ring of aux-plane slots per stream
 constexpr int STAGE_WARPS = STAGE_THREADS / 32;
-constexpr int STREAMS_PER_BLOCK = 2 * STAGE_WARPS;
 
 // Shared memory of one stream.  Plane slot: (8+2R) rows (x) of PY values, the tile at rows/cols R..R+7 and
 // the star halo around it.  For 8-byte values and R = 2 the pitch is 14 so that the two row groups of a
@@ -133,21 +132,25 @@ template <> struct KW<float> {
 
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
 
-template <typename T, int R, int MODE>
-__global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage_kernel(const __grid_constant__ StageParams p) {
+template <typename T, int R, int MODE, int PR>
+__global__ void __launch_bounds__(STAGE_THREADS, (PR == 2 ? 4 : (sizeof(T) == 8 ? 3 : 4)))
+stage_kernel(const __grid_constant__ StageParams p) {
     using C = typename CxOf<T>::type;
     constexpr bool HAS_AUX = mode_has_aux(MODE);
     using G = Geo<T, R, HAS_AUX>;
     constexpr unsigned ES = G::ES;
-    constexpr int NHE = 2 * R;                             // halo values per lane and plane
+    constexpr int LPS = 64 / PR;                           // lanes per stream (16: half-warp, 32: warp)
+    constexpr int SPW = 32 / LPS;                          // streams per warp
+    constexpr int LPH = LPS / 4;                           // lanes per halo side
+    constexpr int NHE = 8 * R / LPH;                       // halo values per lane and plane
     constexpr unsigned SLOT_BYTES = (unsigned)G::PLANE * ES;
     constexpr unsigned ROW_BYTES = (unsigned)G::PY * ES;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int half = lane >> 4, t = lane & 15;
-    const int g = t >> 3, ly = t & 7;                      // row group and column of the 4x1 patch
-    const int sidx = (blockIdx.x * STAGE_WARPS + warp) * 2 + half;   // this half-warp's stream
+    const int half = lane / LPS, t = lane % LPS;
+    const int g = t >> 3, ly = t & 7;                      // row group and column of the PRx1 patch
+    const int sidx = (blockIdx.x * STAGE_WARPS + warp) * SPW + half;   // this (half-)warp's stream
     const bool valid = sidx < p.n_work;
     const WorkRec* __restrict__ w = p.work + (valid ? sidx : 0);
 
@@ -155,12 +158,12 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
     const int kstart = z0 - R;
     const int ne = nz > 0 ? nz + 2 * R : 0;                // planes kstart .. kstart+ne-1 are touched
 
-    const unsigned sb = (unsigned)__cvta_generic_to_shared(smem_raw) + (unsigned)((warp * 2 + half) * G::STREAM_BYTES);
+    const unsigned sb = (unsigned)__cvta_generic_to_shared(smem_raw) + (unsigned)((warp * SPW + half) * G::STREAM_BYTES);
     const unsigned ring = sb, auxring = sb + G::RING_BYTES, smask = sb + G::MASK_OFF, sbase = sb + G::BASE_OFF;
 
     // ---- slab tables of the five tiles -> shared memory (all loads in flight at once) ----------------
     {
-        constexpr int NM = (G::NE + 15) / 16;
+        constexpr int NM = (G::NE + LPS - 1) / LPS;
         unsigned tl[5 * NM], th[5 * NM], tb[5 * NM];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
@@ -168,7 +171,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
             const Slab* __restrict__ tab = p.slabs + w->eoff[q];
 #pragma unroll
             for (int m = 0; m < NM; ++m) {
-                const int i = t + 16 * m, zp = kstart + i;
+                const int i = t + LPS * m, zp = kstart + i;
                 tl[q * NM + m] = 0u; th[q * NM + m] = 0u; tb[q * NM + m] = 0u;
                 if (i < ne && zp >= zl && zp < zh) {
                     const uint4 s = __ldg(reinterpret_cast<const uint4*>(tab + zp));
@@ -180,7 +183,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
         for (int q = 0; q < 5; ++q)
 #pragma unroll
             for (int m = 0; m < NM; ++m) {
-                const int i = t + 16 * m;
+                const int i = t + LPS * m;
                 if (i < G::NE) {
                     sts_u2(smask + (unsigned)((q * G::NE + i) * 8), tl[q * NM + m], th[q * NM + m]);
                     sts_u1(sbase + (unsigned)((q * G::NE + i) * 4), tb[q * NM + m]);
@@ -189,17 +192,21 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
     }
 
     // ---- lane constants ---------------------------------------------------------------------------------
-    unsigned bm[4];                                        // bits below own element e inside its word
+    const bool ghi = PR * g >= 4;                          // own rows live in the high mask word
+    const int rb0 = ((PR * g) & 3) * 8 + ly;               // bit of own element 0 inside its word
+    const unsigned rowmask = PR == 4 ? 0xffffffffu : (0xffffu << (rb0 - ly));   // own rows inside the word
+    unsigned bm[PR];                                       // bits below own element e inside its word
 #pragma unroll
-    for (int e = 0; e < 4; ++e) bm[e] = (1u << (8 * e + ly)) - 1u;
-    const unsigned own_off = (unsigned)G::at(4 * g, ly) * ES;          // + e * ROW_BYTES
-    const unsigned aux_off = (unsigned)(32 * g + ly) * ES;             // + e * 8 * ES
-    // halo duty: neighbour tile hq (0..3 = -x,+x,-y,+y), values 4e + j of its 8R-value edge
-    const int hq = t >> 2, hj = t & 3;
+    for (int e = 0; e < PR; ++e) bm[e] = (1u << (rb0 + 8 * e)) - 1u;
+    const unsigned own_off = (unsigned)G::at(PR * g, ly) * ES;         // + e * ROW_BYTES
+    const unsigned aux_off = (unsigned)(8 * PR * g + ly) * ES;         // + e * 8 * ES
+    // halo duty: neighbour tile hq (0..3 = -x,+x,-y,+y), values LPH*e + hj of its 8R-value edge
+    const int hq = t / LPH, hj = t % LPH;
     unsigned hbm[NHE], hoff[NHE];
+    bool hhi[NHE];                                         // value e lives in the high mask word
 #pragma unroll
     for (int e = 0; e < NHE; ++e) {
-        const int idx = 4 * e + hj;
+        const int idx = LPH * e + hj;
         int nlx, nly, drow, dcol;
         if (hq < 2) {
             const int rr = idx >> 3, cc = idx & 7;
@@ -211,21 +218,21 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
             drow = rr; dcol = hq == 2 ? cc - R : 8 + cc;
         }
         hbm[e] = (1u << ((nlx * 8 + nly) & 31)) - 1u;
+        hhi[e] = nlx >= 4;
         hoff[e] = (unsigned)((drow + R) * G::PY + (dcol + R)) * ES;
     }
-    const bool selA = hq == 0, selB = hq != 1;             // word (hi?) of values e < NHE/2 and e >= NHE/2
 
     const C* __restrict__ in = reinterpret_cast<const C*>(p.in);
     const C* __restrict__ auxp = reinterpret_cast<const C*>(p.aux);
 
     // potential: u = qxy[e] + qz(plane); qxy = 1/2 (ax x^2 + ay y^2) of the patch points
-    double qxy[4];
+    double qxy[PR];
     {
         const double y = ((double)(w->iy0 + ly) - p.yc) * p.pot.h + p.pot.cy;
         const double qy = p.hay * (y * y);
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const double x = ((double)(w->ix0 + 4 * g + e) - p.xc) * p.pot.h + p.pot.cx;
+        for (int e = 0; e < PR; ++e) {
+            const double x = ((double)(w->ix0 + PR * g + e) - p.xc) * p.pot.h + p.pot.cx;
             qxy[e] = fma(p.hax, x * x, qy);
         }
     }
@@ -233,7 +240,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
     if (MODE == MODE_IMAG) { sc = *p.scale_in; gsc = p.g * (sc * sc); }
 
     int niter = ne;
-    niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16));   // both halves run the same loop
+    if (SPW == 2) niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16));   // both halves run the same loop
     __syncwarp();                                                  // tables visible to the half-warp
 
     // ---- producer: plane index i (plane kstart + i) -> slot sp; aux of plane i - R -> aux slot ap ------
@@ -241,12 +248,12 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
         if (i < ne) {
             {
                 const uint2 m = lds_u2(smask + (unsigned)i * 8u);
-                const unsigned word = g ? m.y : m.x;
-                const unsigned bc = lds_u1(sbase + (unsigned)i * 4u) + (g ? (unsigned)__popc(m.x) : 0u);
+                const unsigned word = ghi ? m.y : m.x;
+                const unsigned bc = lds_u1(sbase + (unsigned)i * 4u) + (ghi ? (unsigned)__popc(m.x) : 0u);
                 const unsigned dst = ring + sp * SLOT_BYTES + own_off;
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const bool on = (word >> (8 * e + ly)) & 1u;
+                for (int e = 0; e < PR; ++e) {
+                    const bool on = (word >> (rb0 + 8 * e)) & 1u;
                     cp_async_zfill(dst + (unsigned)e * ROW_BYTES, in + (bc + (unsigned)__popc(word & bm[e])), on);
                 }
             }
@@ -255,12 +262,10 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
                 const uint2 m = lds_u2(smask + ti * 8u);
                 const unsigned b = lds_u1(sbase + ti * 4u);
                 const unsigned pl = (unsigned)__popc(m.x);
-                const unsigned wA = selA ? m.y : m.x, wB = selB ? m.y : m.x;
-                const unsigned bA = b + (selA ? pl : 0u), bB = b + (selB ? pl : 0u);
                 const unsigned dst = ring + sp * SLOT_BYTES;
 #pragma unroll
                 for (int e = 0; e < NHE; ++e) {
-                    const unsigned ww = e < NHE / 2 ? wA : wB, bb = e < NHE / 2 ? bA : bB;
+                    const unsigned ww = hhi[e] ? m.y : m.x, bb = b + (hhi[e] ? pl : 0u);
                     const bool on = (ww & (hbm[e] + 1u)) != 0u;
                     cp_async_zfill(dst + hoff[e], in + (bb + (unsigned)__popc(ww & hbm[e])), on);
                 }
@@ -269,12 +274,12 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
                 const int ia = i - R;
                 if (ia >= R && ia < ne - R) {
                     const uint2 m = lds_u2(smask + (unsigned)ia * 8u);
-                    const unsigned word = g ? m.y : m.x;
-                    const unsigned bc = lds_u1(sbase + (unsigned)ia * 4u) + (g ? (unsigned)__popc(m.x) : 0u);
+                    const unsigned word = ghi ? m.y : m.x;
+                    const unsigned bc = lds_u1(sbase + (unsigned)ia * 4u) + (ghi ? (unsigned)__popc(m.x) : 0u);
                     const unsigned dst = auxring + ap * (64u * ES) + aux_off;
 #pragma unroll
-                    for (int e = 0; e < 4; ++e)
-                        if ((word >> (8 * e + ly)) & 1u)
+                    for (int e = 0; e < PR; ++e)
+                        if ((word >> (rb0 + 8 * e)) & 1u)
                             cp_async_zfill(dst + (unsigned)e * (8u * ES), auxp + (bc + (unsigned)__popc(word & bm[e])), true);
                 }
             }
@@ -283,11 +288,11 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
     };
 
     // state (accumulate-forward form): set s holds psi and the partial T psi of one earlier plane
-    C SP[R][4], SA[R][4];
+    C SP[R][PR], SA[R][PR];
 #pragma unroll
     for (int s = 0; s < R; ++s)
 #pragma unroll
-        for (int e = 0; e < 4; ++e) { SP[s][e] = mk<T>((T)0, (T)0); SA[s][e] = mk<T>((T)0, (T)0); }
+        for (int e = 0; e < PR; ++e) { SP[s][e] = mk<T>((T)0, (T)0); SA[s][e] = mk<T>((T)0, (T)0); }
     double acc[NACC] = {0.0, 0.0, 0.0, 0.0};
 
     // ---- prologue: planes 0 .. PF-1 in flight ----------------------------------------------------------------
@@ -296,7 +301,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
 
     // one plane step at plane index i (plane k = kstart + i).  (PN, AN) = set of plane k-1, (PO, AO) = set of
     // plane k-R (the same set for R = 1).  sl = ring slot of plane i; al = aux slot of plane i - R.
-    auto step = [&](C (&PN)[4], C (&AN)[4], C (&PO)[4], C (&AO)[4], const int i, const unsigned sl, const unsigned al) {
+    auto step = [&](C (&PN)[PR], C (&AN)[PR], C (&PO)[PR], C (&AO)[PR], const int i, const unsigned sl, const unsigned al) {
         cp_async_wait<PF - 1>();
         __syncwarp();
         {
@@ -312,16 +317,16 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
         unsigned cword = 0u, cbase = 0u;
         if (ic >= R) {
             const uint2 m = lds_u2(smask + (unsigned)ic * 8u);
-            cword = g ? m.y : m.x;
-            cbase = lds_u1(sbase + (unsigned)ic * 4u) + (g ? (unsigned)__popc(m.x) : 0u);
+            cword = ghi ? m.y : m.x;
+            cbase = lds_u1(sbase + (unsigned)ic * 4u) + (ghi ? (unsigned)__popc(m.x) : 0u);
         }
         // ---- psi(k) of the patch ------------------------------------------------------------------------
-        C v[4];
+        C v[PR];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) v[e] = lds_c(so + (unsigned)e * ROW_BYTES, (C*)nullptr);
+        for (int e = 0; e < PR; ++e) v[e] = lds_c(so + (unsigned)e * ROW_BYTES, (C*)nullptr);
         // ---- psi(k) completes the z part of planes k-1 .. k-R -------------------------------------------
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
+        for (int e = 0; e < PR; ++e) {
             AO[e].x = fma(KW<T>::w(p, R), v[e].x, AO[e].x);
             AO[e].y = fma(KW<T>::w(p, R), v[e].y, AO[e].y);
             if (R == 2) {
@@ -330,12 +335,12 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
             }
         }
         // ---- finish plane c = k - R: V(r,t), nonlinear term, stage combination --------------------------------
-        if (cword) {
+        if (cword & rowmask) {
             const double zc = ((double)(kstart + ic) - p.zc) * p.pot.h + p.pot.cz;
             const double qz = p.haz * (zc * zc) - p.delta_eff;
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const bool on = (cword >> (8 * e + ly)) & 1u;
+            for (int e = 0; e < PR; ++e) {
+                const bool on = (cword >> (rb0 + 8 * e)) & 1u;
                 const unsigned pos = cbase + (unsigned)__popc(cword & bm[e]);
                 const C cv = PO[e];
                 const C tc = AO[e];
@@ -384,7 +389,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
         }
         // ---- the oldest set becomes the set of plane k: z-backward part, centre ---------------------------------
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
+        for (int e = 0; e < PR; ++e) {
             C an;
             if (R == 2) {
                 an.x = KW<T>::w(p, 2) * PO[e].x;
@@ -401,12 +406,12 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
         }
         // ---- in-plane part (only planes of the stream itself are ever finished) ----------------------------------
         if (i >= R && i < ne - R) {
-            // x direction: source rows r = -R .. 3+R of column ly; rows 0..3 are the patch itself
+            // x direction: source rows r = -R .. PR-1+R of column ly; rows 0..PR-1 are the patch itself
 #pragma unroll
-            for (int r = -R; r <= 3 + R; ++r) {
-                const C val = (r >= 0 && r <= 3) ? v[r] : lds_c(so + (unsigned)(r * (int)ROW_BYTES), (C*)nullptr);
+            for (int r = -R; r <= PR - 1 + R; ++r) {
+                const C val = (r >= 0 && r < PR) ? v[r < 0 ? 0 : (r < PR ? r : 0)] : lds_c(so + (unsigned)(r * (int)ROW_BYTES), (C*)nullptr);
 #pragma unroll
-                for (int a = 0; a < 4; ++a) {
+                for (int a = 0; a < PR; ++a) {
                     const int d = r > a ? r - a : a - r;
                     if (d >= 1 && d <= R) {
                         AO[a].x = fma(KW<T>::w(p, d), val.x, AO[a].x);
@@ -416,7 +421,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
             }
             // y direction: columns ly +- 1 .. R of each patch row
 #pragma unroll
-            for (int a = 0; a < 4; ++a) {
+            for (int a = 0; a < PR; ++a) {
 #pragma unroll
                 for (int cc = -R; cc <= R; ++cc) {
                     if (cc == 0) continue;
@@ -453,7 +458,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
 #pragma unroll
         for (int kq = 0; kq < NACC; ++kq)
 #pragma unroll
-            for (int off = 8; off > 0; off >>= 1) acc[kq] += __shfl_down_sync(0xffffffffu, acc[kq], off, 16);
+            for (int off = LPS / 2; off > 0; off >>= 1) acc[kq] += __shfl_down_sync(0xffffffffu, acc[kq], off, LPS);
         if (t == 0 && valid) {
 #pragma unroll
             for (int kq = 0; kq < NACC; ++kq) p.partials[(size_t)sidx * NACC + kq] = acc[kq];
@@ -461,14 +466,19 @@ __global__ void __launch_bounds__(STAGE_THREADS, (sizeof(T) == 8 ? 3 : 4)) stage
     }
 }
 
+// rows per lane: complex128 lanes carry 2 rows (a warp per stream: half the registers, twice the resident
+// warps), complex64 lanes 4 rows (a half-warp per stream)
+template <typename T> constexpr int rows_per_lane() { return sizeof(T) == 8 ? 2 : 4; }
+
 template <typename T, int R, int MODE> constexpr size_t stage_smem() {
-    return (size_t)STREAMS_PER_BLOCK * Geo<T, R, mode_has_aux(MODE)>::STREAM_BYTES;
+    return (size_t)(STAGE_WARPS * rows_per_lane<T>() / 2) * Geo<T, R, mode_has_aux(MODE)>::STREAM_BYTES;
 }
 
 template <typename T, int R, int MODE>
 cudaError_t launch_one(const StageParams& p, cudaStream_t st) {
-    const int nblk = (p.n_work + STREAMS_PER_BLOCK - 1) / STREAMS_PER_BLOCK;
-    stage_kernel<T, R, MODE><<<nblk, STAGE_THREADS, stage_smem<T, R, MODE>(), st>>>(p);
+    constexpr int spb = STAGE_WARPS * rows_per_lane<T>() / 2;   // streams per block
+    const int nblk = (p.n_work + spb - 1) / spb;
+    stage_kernel<T, R, MODE, rows_per_lane<T>()><<<nblk, STAGE_THREADS, stage_smem<T, R, MODE>(), st>>>(p);
     return cudaGetLastError();
 }
 
@@ -488,7 +498,7 @@ cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
 
 template <typename T, int R, int MODE>
 cudaError_t set_attr() {
-    return cudaFuncSetAttribute(stage_kernel<T, R, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    return cudaFuncSetAttribute(stage_kernel<T, R, MODE, rows_per_lane<T>()>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)stage_smem<T, R, MODE>());
 }
 template <typename T, int R>

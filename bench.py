@@ -183,6 +183,27 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+def aggregate_replicas(ms, n, device=None):
+    """Whole-job figures of N independent replicas (replicas only, no data-path
+    collective): the timed region is as long as the slowest rank's (MAX), the work is the sum of the ranks'
+    active points (SUM).  Works on any initialised torch.distributed backend (nccl on the GPU box, gloo in the
+    CPU tests); without a process group it is the identity."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms), float(n)
+    t = torch.tensor([float(ms)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([float(n)], device=device, dtype=torch.float64)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(c.item())
+
+
+def stage_updates_per_s(n_all, steps, ms):
+    """BASELINE metric: active-point RK4 stage updates per second (4 stage updates per point and step)."""
+    return n_all * 4 * steps / (ms * 1e-3)
+
+
 def run_ours(args, w):
     import torch
     import torch.distributed as dist
@@ -241,16 +262,8 @@ def run_ours(args, w):
     stage_ms, stage_cnt = sim.stage_time_ms()
     sim.time_stages(False)
     launches = sim.kernel_launches - l0
-    if world > 1:
-        tmax = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms = float(tmax.item())
-        ntot = torch.tensor([n], device=dev, dtype=torch.float64)
-        dist.all_reduce(ntot, op=dist.ReduceOp.SUM)
-        n_all = float(ntot.item())
-    else:
-        n_all = float(n)
-    value = n_all * 4 * args.steps / (ms * 1e-3)
+    ms, n_all = aggregate_replicas(ms, n, dev)
+    value = stage_updates_per_s(n_all, args.steps, ms)
     nrm = sim.norm()
     if not (abs(nrm - 1.0) < 1e-2):
         raise SystemExit(f"bench.py: state lost normalisation ({nrm}); the run is invalid")
@@ -292,10 +305,7 @@ def run_ours(args, w):
         sim.get_psi_host(out_np)
     torch.cuda.synchronize(dev)
     t_e2e = time.perf_counter() - t0
-    if world > 1:
-        tt = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_e2e = float(tt.item())
+    t_e2e, _ = aggregate_replicas(t_e2e, n, dev)
     e2e = {"value": n_all * 4 * e2e_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": n * csize,
            "d2h_bytes_per_step": n * csize, "steps": e2e_steps,
            "call": "gpe_set_psi_host + gpe_run_rk4(1) + gpe_get_psi_host per step, pinned host buffers"}

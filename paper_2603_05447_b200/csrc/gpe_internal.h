@@ -92,7 +92,7 @@ enum Mode : int {
     MODE_ENERGY = 6  // partial sums of Re(conj(c) T c), V|c|^2, |c|^4, |c|^2
 };
 constexpr int NACC = 4;           // accumulators per block in the partial-sum array
-constexpr int STAGE_THREADS = 128;
+constexpr int STAGE_THREADS = 32;
 
 struct StageParams {
     const Slab* slabs;

@@ -82,16 +82,15 @@ __device__ __forceinline__ void sts_u1(unsigned addr, unsigned a) {
     asm volatile("st.shared.u32 [%0], %1;\n" ::"r"(addr), "r"(a) : "memory");
 }
 
-// sqrt(s) for s >= 0 from the hardware reciprocal-square-root seed and two coupled Newton steps
-// (relative error a few 1e-16; the IEEE-rounded sqrt() costs about twice the FP64 instructions).
+// sqrt(s) for s >= 0 from the hardware reciprocal-square-root seed (about 2^-23 relative), one coupled
+// Newton step for g ~ sqrt(s) and h ~ 1/(2 sqrt(s)) (2^-45) and the residual correction g + (s - g^2) h, whose
+// error is second order in the 2^-45 (relative error a few 1e-16 from rounding only; the IEEE-rounded sqrt()
+// costs about three times the FP64 instructions).
 __device__ __forceinline__ double fast_sqrt(double s) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;\n" : "=d"(y) : "d"(s));
     double g = s * y, h = 0.5 * y;
     double r = fma(-g, h, 0.5);
-    g = fma(g, r, g);
-    h = fma(h, r, h);
-    r = fma(-g, h, 0.5);
     g = fma(g, r, g);
     h = fma(h, r, h);
     r = fma(-g, g, s);          // residual s - g^2
@@ -133,7 +132,7 @@ template <> struct KW<float> {
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
 
 template <typename T, int R, int MODE, int PR>
-__global__ void __launch_bounds__(STAGE_THREADS, (PR == 2 ? 4 : (sizeof(T) == 8 ? 3 : 4)))
+__global__ void __launch_bounds__(STAGE_THREADS, (PR == 2 ? 16 : (sizeof(T) == 8 ? 12 : 16)))
 stage_kernel(const __grid_constant__ StageParams p) {
     using C = typename CxOf<T>::type;
     constexpr bool HAS_AUX = mode_has_aux(MODE);
@@ -194,7 +193,6 @@ stage_kernel(const __grid_constant__ StageParams p) {
     // ---- lane constants ---------------------------------------------------------------------------------
     const bool ghi = PR * g >= 4;                          // own rows live in the high mask word
     const int rb0 = ((PR * g) & 3) * 8 + ly;               // bit of own element 0 inside its word
-    const unsigned rowmask = PR == 4 ? 0xffffffffu : (0xffffu << (rb0 - ly));   // own rows inside the word
     unsigned bm[PR];                                       // bits below own element e inside its word
 #pragma unroll
     for (int e = 0; e < PR; ++e) bm[e] = (1u << (rb0 + 8 * e)) - 1u;
@@ -315,15 +313,30 @@ stage_kernel(const __grid_constant__ StageParams p) {
         const int ic = i - R;                                   // plane finished in this step
         // ---- output plane: activity bits and storage positions --------------------------------------------
         unsigned cword = 0u, cbase = 0u;
+        bool cany = false;                                      // the slab of plane c holds points (stream-uniform)
         if (ic >= R) {
             const uint2 m = lds_u2(smask + (unsigned)ic * 8u);
             cword = ghi ? m.y : m.x;
             cbase = lds_u1(sbase + (unsigned)ic * 4u) + (ghi ? (unsigned)__popc(m.x) : 0u);
+            cany = (m.x | m.y) != 0u;
         }
         // ---- psi(k) of the patch ------------------------------------------------------------------------
         C v[PR];
 #pragma unroll
         for (int e = 0; e < PR; ++e) v[e] = lds_c(so + (unsigned)e * ROW_BYTES, (C*)nullptr);
+        // ---- V(r,t) of plane c: depends on coordinates only, so its dependency chains (one per patch point,
+        //      interleaved) are issued here and overlap the shared-memory latency of psi(k) --------------------
+        double vpot[PR];
+        if (cany) {
+            const double zc = ((double)(kstart + ic) - p.zc) * p.pot.h + p.pot.cz;
+            const double qz = p.haz * (zc * zc) - p.delta_eff;
+#pragma unroll
+            for (int e = 0; e < PR; ++e) vpot[e] = qxy[e] + qz;
+            if (p.pot.kind == GPE_POT_DRESSED) {
+#pragma unroll
+                for (int e = 0; e < PR; ++e) vpot[e] = fast_sqrt(fma(vpot[e], vpot[e], p.om2)) - p.pot.omega;
+            }
+        }
         // ---- psi(k) completes the z part of planes k-1 .. k-R -------------------------------------------
 #pragma unroll
         for (int e = 0; e < PR; ++e) {
@@ -334,31 +347,30 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 AN[e].y = fma(KW<T>::w(p, 1), v[e].y, AN[e].y);
             }
         }
-        // ---- finish plane c = k - R: V(r,t), nonlinear term, stage combination --------------------------------
-        if (cword & rowmask) {
-            const double zc = ((double)(kstart + ic) - p.zc) * p.pot.h + p.pot.cz;
-            const double qz = p.haz * (zc * zc) - p.delta_eff;
+        // ---- finish plane c = k - R: nonlinear term, stage combination (branch-free; stores predicated) ----
+        if (cany) {
+            C av[PR];
+#pragma unroll
+            for (int e = 0; e < PR; ++e) {
+                av[e] = mk<T>((T)0, (T)0);
+                if (HAS_AUX) av[e] = lds_c(auxring + al * (64u * ES) + aux_off + (unsigned)e * (8u * ES), (C*)nullptr);
+            }
 #pragma unroll
             for (int e = 0; e < PR; ++e) {
                 const bool on = (cword >> (rb0 + 8 * e)) & 1u;
                 const unsigned pos = cbase + (unsigned)__popc(cword & bm[e]);
                 const C cv = PO[e];
                 const C tc = AO[e];
-                C av = mk<T>((T)0, (T)0);
-                if (HAS_AUX) av = lds_c(auxring + al * (64u * ES) + aux_off + (unsigned)e * (8u * ES), (C*)nullptr);
-                double vpot = qxy[e] + qz;
-                if (p.pot.kind == GPE_POT_DRESSED) vpot = fast_sqrt(fma(vpot, vpot, p.om2)) - p.pot.omega;
                 const T a2 = fma(cv.x, cv.x, cv.y * cv.y);
                 if (MODE == MODE_ENERGY) {
-                    if (on) {
-                        acc[0] += (double)(cv.x * tc.x + cv.y * tc.y);
-                        acc[1] += vpot * (double)a2;
-                        acc[2] += (double)a2 * (double)a2;
-                        acc[3] += (double)a2;
-                    }
+                    // inactive lanes hold cv = 0 and finite tc: they add exact zeros
+                    acc[0] += (double)(cv.x * tc.x + cv.y * tc.y);
+                    acc[1] += vpot[e] * (double)a2;
+                    acc[2] += (double)a2 * (double)a2;
+                    acc[3] += (double)a2;
                     continue;
                 }
-                const T diag = (T)fma(gsc, (double)a2, vpot);
+                const T diag = (T)fma(gsc, (double)a2, vpot[e]);
                 const C hc = mk<T>(fma(diag, cv.x, tc.x), fma(diag, cv.y, tc.y));
                 const T ca = (T)p.ca;
                 C o;
@@ -367,10 +379,11 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 } else if (MODE == MODE_IMAG) {
                     const T s = (T)sc;
                     o = mk<T>(s * fma(-ca, hc.x, cv.x), s * fma(-ca, hc.y, cv.y));
-                    if (on) acc[0] += (double)o.x * (double)o.x + (double)o.y * (double)o.y;
+                    const double o2 = (double)o.x * (double)o.x + (double)o.y * (double)o.y;
+                    acc[0] += on ? o2 : 0.0;
                 } else {
                     // f = -i H c = (hc.y, -hc.x)
-                    const C base = (MODE == MODE_S1) ? cv : av;
+                    const C base = (MODE == MODE_S1) ? cv : av[e];
                     o = mk<T>(fma(ca, hc.y, base.x), fma(-ca, hc.x, base.y));
                     if (MODE == MODE_S4) {
                         const T third = (T)(1.0 / 3.0);
@@ -379,9 +392,8 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     }
                     if (MODE == MODE_S2) {
                         const T third = (T)(1.0 / 3.0), tt = (T)(2.0 / 3.0);
-                        if (on)
-                            reinterpret_cast<C*>(p.out2)[pos] =
-                                mk<T>(fma(tt, o.x, third * (cv.x - av.x)), fma(tt, o.y, third * (cv.y - av.y)));
+                        const C o2 = mk<T>(fma(tt, o.x, third * (cv.x - av[e].x)), fma(tt, o.y, third * (cv.y - av[e].y)));
+                        if (on) reinterpret_cast<C*>(p.out2)[pos] = o2;
                     }
                 }
                 if (on) reinterpret_cast<C*>(p.out1)[pos] = o;

@@ -20,6 +20,11 @@ Pin status (tests/test_oracle_pins.py): coords/potential/mask, apply_T (7 and
 13 pt), apply_H, rk4_step, norm/energy, layout tables: PINNED (P1-P12).
 imag_step for g > 0 and long nonlinear dynamics: "parity unpinned" beyond the
 g = 0 harmonic ground state and monotone-energy invariants (no closed form).
+imag_split_step (the paper's own scheme): PINNED for g = 0 (P13: the
+iteration matrix D K D built from Kronecker products, its top eigenvector and the
+O(dt^2) splitting error of the ground-state energy) and for the one-point mask
+(closed form); for g > 0 "parity unpinned" beyond those and the agreement of its
+fixed point with imag_step's to O(dt).
 """
 from __future__ import annotations
 
@@ -253,6 +258,32 @@ def imag_step(grid, pot, g, t, dt, psi, stencil, n_target=1.0):
 def run_imag(grid, pot, g, t, dt, nsteps, psi, stencil, n_target=1.0):
     for _ in range(nsteps):
         psi = imag_step(grid, pot, g, t, dt, psi, stencil, n_target)
+    return psi
+
+
+def diag_propagator(grid, pot, g, t, dt, psi):
+    """Eq. 7 for half a step with the interaction factor linearised as the paper does:
+    psi -> psi * exp(-V dt/2) * (1 - g |psi|^2 dt/2)   ("the interaction propagator can be approximated as
+    1 - g psi^2 dt / 2 hbar"; hbar = 1)."""
+    v = potential_at(grid.box, pot, grid.active, t)
+    return psi * np.exp(-0.5 * dt * v) * (1.0 - (0.5 * dt * g) * (psi.real ** 2 + psi.imag ** 2))
+
+
+def imag_split_step(grid, pot, g, t, dt, psi, stencil, n_target=1.0):
+    """One iteration of the paper's own ground-state scheme, in its order (PAPER.md:60-67, :87 kernels K1-K3):
+    half a step of the diagonal operators (Eq. 7, linearised interaction), the kinetic propagation for a total
+    time dt "in two steps using the forward Euler method" (two steps of dt/2 each, PAPER.md:67 and footnote
+    [44] at :236), one more Eq. 7 half step, renormalisation to n_target.  V frozen at time t."""
+    p = diag_propagator(grid, pot, g, t, dt, psi)
+    p = p - (0.5 * dt) * apply_T(grid, p, stencil)
+    p = p - (0.5 * dt) * apply_T(grid, p, stencil)
+    p = diag_propagator(grid, pot, g, t, dt, p)
+    return p * math.sqrt(n_target / norm(grid, p))
+
+
+def run_imag_split(grid, pot, g, t, dt, nsteps, psi, stencil, n_target=1.0):
+    for _ in range(nsteps):
+        psi = imag_split_step(grid, pot, g, t, dt, psi, stencil, n_target)
     return psi
 
 

@@ -438,3 +438,87 @@ def test_uniform01_is_layout_independent_and_uniform():
     p = np.random.default_rng(0).permutation(lin.size)
     assert np.array_equal(I.uniform01(3, lin[p]), u[p])
     assert not np.array_equal(I.uniform01(4, lin), u)
+
+
+# ---- P13: the paper's own imaginary-time scheme: D K K D, renormalise -----------------
+def _kron_T(nx, ny, nz, h, stencil, act):
+    eye = np.eye
+    lap = (np.kron(np.kron(lap1d(nx, h, stencil), eye(ny)), eye(nz))
+           + np.kron(np.kron(eye(nx), lap1d(ny, h, stencil)), eye(nz))
+           + np.kron(np.kron(eye(nx), eye(ny)), lap1d(nz, h, stencil)))
+    return -0.5 * lap[np.ix_(act, act)]
+
+
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_P13_split_step_is_DKKD_matrix_at_g0(stencil):
+    """g = 0: one iteration is the matrix M = D (1 - dt/2 T)^2 D, D = diag exp(-V dt/2), applied and
+    normalised; T from Kronecker products with rows / columns deleted, V from the coordinates."""
+    nx, ny, nz, h, dt = 6, 5, 7, 0.6, 0.02
+    act = I.random_mask_lin(11, nx, ny, nz, 0.7)
+    box = O.Box(nx, ny, nz, h)
+    grid = O.SparseGrid(box, act, 2)
+    pot = O.Potential(kind=O.HARMONIC, ax=1.0, ay=2.0, az=0.5)
+    ix, iy, iz = act // (ny * nz), (act // nz) % ny, act % nz
+    x, y, z = (ix - 0.5 * (nx - 1)) * h, (iy - 0.5 * (ny - 1)) * h, (iz - 0.5 * (nz - 1)) * h
+    d = np.exp(-0.5 * dt * 0.5 * (1.0 * x * x + 2.0 * y * y + 0.5 * z * z))
+    k = np.eye(act.size) - 0.5 * dt * _kron_T(nx, ny, nz, h, stencil, act)
+    m = np.diag(d) @ k @ k @ np.diag(d)
+    assert np.max(np.abs(m - m.T)) < 1e-14                      # symmetric: a power iteration
+    psi = I.random_psi(12, act.size)
+    want = m @ psi
+    want = want / math.sqrt(h ** 3 * np.sum(np.abs(want) ** 2))
+    got = O.imag_split_step(grid, pot, 0.0, 0.0, dt, psi, stencil)
+    assert np.max(np.abs(got - want)) < 1e-13 * np.max(np.abs(want)) * 10
+    # fixed point = top eigenvector of M
+    ev, evec = np.linalg.eigh(m)
+    top = evec[:, -1] * np.sign(evec[np.argmax(np.abs(evec[:, -1])), -1])
+    top = top / math.sqrt(h ** 3 * np.sum(top ** 2))
+    psi = np.abs(psi.real).astype(np.complex128) + 0.1
+    psi = O.run_imag_split(grid, pot, 0.0, 0.0, dt, 4000, psi, stencil)
+    assert np.max(np.abs(psi - top)) < 1e-9 * np.max(np.abs(top))
+
+
+def test_P13_split_scheme_ground_state_energy_error_is_second_order_in_dt():
+    """Symmetric splitting: the energy of the fixed point differs from the discrete ground-state energy by
+    O(dt^2) (the first-order term cancels between the two half steps); halving dt divides the error by 4."""
+    n, h = 10, 0.7
+    box, grid = full_box_grid(n, n, n, h)
+    act = np.arange(n ** 3)
+    pot = O.Potential(kind=O.HARMONIC)
+    e1, _ = ho_ground_state_1d(n, h, 7)
+    x = O.coords(n, h)
+    v = 0.5 * (x[:, None, None] ** 2 + x[None, :, None] ** 2 + x[None, None, :] ** 2).ravel()
+    tm = _kron_T(n, n, n, h, 7, act)
+    errs = []
+    for dt in (0.08, 0.04):
+        d = np.exp(-0.5 * dt * v)
+        k = np.eye(n ** 3) - 0.5 * dt * tm
+        m = (d[:, None] * (k @ k)) * d[None, :]
+        ev, evec = np.linalg.eigh(m)
+        top = np.abs(evec[:, -1]).astype(np.complex128)
+        top /= math.sqrt(O.norm(grid, top))
+        # the oracle's iteration has that fixed point ...
+        assert np.max(np.abs(O.imag_split_step(grid, pot, 0.0, 0.0, dt, top, 7) - top)) < 1e-12
+        # ... whose energy is off by O(dt^2)
+        errs.append(O.energy(grid, pot, 0.0, 0.0, top, 7)["total"] - 3 * e1)
+    assert errs[0] > errs[1] > 0
+    assert 3.5 < errs[0] / errs[1] < 4.5
+
+
+def test_P13_linearised_interaction_factor():
+    """exp(-g|psi|^2 dt/2) approximated as 1 - g|psi|^2 dt/2: the oracle's factor differs from the
+    exponential one by x^2/2 - x^3/6 + ... with x = g |psi|^2 dt / 2, point by point."""
+    w = I.small_shell(24, 7)
+    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center)
+    pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
+    act = O.active_indices(box, pot, w.v_cut, w.mask_mode)
+    grid = O.SparseGrid(box, act, 1)
+    psi = I.make_psi0(w, act)
+    g, dt = 3.0e4, 0.01
+    x = g * np.abs(psi) ** 2 * dt / 2
+    assert 0.01 < x.max() < 0.5
+    exact = psi * np.exp(-0.5 * dt * O.potential_at(box, pot, act, 0.0)) * np.exp(-x)
+    lin = O.diag_propagator(grid, pot, g, 0.0, dt, psi)
+    ratio = lin / exact                                        # = (1 - x) e^{x} = 1 - x^2/2 - x^3/3 - ...
+    assert np.max(np.abs(ratio - (1 - x) * np.exp(x))) < 1e-14
+    assert np.all(ratio.real <= 1.0) and np.max(np.abs(1 - ratio.real - x ** 2 / 2)) < x.max() ** 3

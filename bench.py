@@ -326,6 +326,8 @@ def run_ours(args, w):
     extra = {"layout_build_s": t_layout, "n_tiles": info.n_tiles, "n_work_items": info.n_work}
     ms_imag = timed(lambda: sim.run_imag(w.dt, 10), 2) / 10
     extra["imag_step"] = {"ms": ms_imag, "point_updates_per_s": n / (ms_imag * 1e-3), "GBps": 2 * csize * n / (ms_imag * 1e-3) / 1e9}
+    ms_sp = timed(lambda: sim.run_imag_split(w.dt, 10), 2) / 10
+    extra["imag_split_step"] = {"ms": ms_sp, "point_updates_per_s": n / (ms_sp * 1e-3), "GBps": 6 * csize * n / (ms_sp * 1e-3) / 1e9}
     ms_en = timed(lambda: sim.energy(), 3)
     extra["energy"] = {"ms": ms_en, "GBps": csize * n / (ms_en * 1e-3) / 1e9}
     ms_nm = timed(lambda: sim.norm(), 3)

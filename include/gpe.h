@@ -184,6 +184,20 @@ int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 int gpe_imag_step(gpe_sim* s, double dt, void* stream);
 int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 
+/* a5 (second mode): the paper's own ground-state iteration, in its order (PAPER.md:60-67,
+ * :87 kernels K1-K3, footnote [44] at :236), V frozen at the sim clock:
+ *   psi <- psi exp(-V dt/2) (1 - g |psi|^2 dt/2)        Eq. 7 for dt/2, interaction factor linearised (:67)
+ *   psi <- psi - (dt/2) T psi, twice                     kinetic propagation for dt "in two steps using the
+ *                                                        forward Euler method"
+ *   psi <- psi exp(-V dt/2) (1 - g |psi|^2 dt/2)        Eq. 7 once more
+ *   psi <- psi sqrt(n_target / (h^3 sum |psi|^2))        renormalisation
+ * Three stage launches per iteration (pointwise Eq. 7 with the lazily applied scale of the previous iteration;
+ * Euler half step; Euler half step + Eq. 7 + block partial sums) and a one-block finalise; exp(-V dt/2) is
+ * evaluated analytically per point (no propagator array is read).  The scale is flushed at the end of the call.
+ * psi stays complex (the real-valued variant of :67 is not built).  Same arguments and errors as gpe_run_imag. */
+int gpe_imag_split_step(gpe_sim* s, double dt, void* stream);
+int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream);
+
 /* a6: reductions over the sim's psi; fp64 accumulation, fixed summation order (bit-reproducible).
  * Synchronise `stream`.  Energy terms use V at the sim clock. */
 int gpe_norm(gpe_sim* s, double* out_host, void* stream);

@@ -62,7 +62,7 @@ SYMBOLS = (
     "gpe_sim_destroy", "gpe_set_psi", "gpe_get_psi", "gpe_set_psi_host", "gpe_get_psi_host",
     "gpe_set_time", "gpe_get_time", "gpe_apply_H", "gpe_step_rk4", "gpe_run_rk4", "gpe_imag_step",
     "gpe_run_imag", "gpe_norm", "gpe_energy", "gpe_sim_kernel_launches", "gpe_sim_time_stages",
-    "gpe_sim_stage_time_ms", "gpe_sim_set_planes_per_block",
+    "gpe_sim_stage_time_ms", "gpe_sim_set_planes_per_block", "gpe_imag_split_step", "gpe_run_imag_split",
 )
 
 _lib = None
@@ -269,6 +269,12 @@ class Sim:
 
     def run_imag(self, dt, nsteps, stream=None):
         _check(lib().gpe_run_imag(self._h, C.c_double(dt), C.c_int64(nsteps), _stream_ptr(stream)))
+
+    def imag_split_step(self, dt, stream=None):
+        _check(lib().gpe_imag_split_step(self._h, C.c_double(dt), _stream_ptr(stream)))
+
+    def run_imag_split(self, dt, nsteps, stream=None):
+        _check(lib().gpe_run_imag_split(self._h, C.c_double(dt), C.c_int64(nsteps), _stream_ptr(stream)))
 
     # -- reductions (synchronise the stream) ------------------------------------------------------------
     def norm(self, stream=None) -> float:

@@ -492,6 +492,30 @@ int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
 
 int gpe_imag_step(gpe_sim* s, double dt, void* stream) { return gpe_run_imag(s, dt, 1, stream); }
 
+int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
+    if (s->n == 0 || nsteps == 0) return GPE_OK;
+    const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;
+    const double hdt = 0.5 * dt;
+    for (int64_t n = 0; n < nsteps; ++n) {
+        // A holds the un-normalised state of the previous iteration; its scale sits in d_sums[NACC]
+        int rc = stage(s, MODE_PREP, s->t, hdt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
+        if (!rc) rc = stage(s, MODE_KIN, s->t, hdt, s->buf[1], nullptr, s->buf[0], nullptr, stream);
+        if (!rc) rc = stage(s, MODE_SPLITB, s->t, hdt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
+        if (rc) return rc;
+        KL(launch_finalize(s->d_partials, s->n_blocks, s->d_sums, s->d_sums + NACC, s->n_target, h3, stream));
+        s->launches += 1;
+        std::swap(s->buf[0], s->buf[1]);
+    }
+    KL(launch_scale(s->dtype, s->buf[0], s->n, s->d_sums + NACC, stream));
+    KL(launch_set_scalar(s->d_sums + NACC, 1.0, stream));
+    s->launches += 2;
+    return GPE_OK;
+}
+
+int gpe_imag_split_step(gpe_sim* s, double dt, void* stream) { return gpe_run_imag_split(s, dt, 1, stream); }
+
 int gpe_norm(gpe_sim* s, double* out_host, void* stream) {
     if (!s || !out_host) return fail(GPE_ERR_INVALID_ARG, "null argument");
     const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;

@@ -89,7 +89,11 @@ enum Mode : int {
     MODE_S3 = 3,     // out1 = aux + ca * f(c)
     MODE_S4 = 4,     // out1 = aux + 1/3 c + ca * f(c)
     MODE_IMAG = 5,   // psi = scale * c; out1 = psi - ca * H psi; partial sum of |out1|^2
-    MODE_ENERGY = 6  // partial sums of Re(conj(c) T c), V|c|^2, |c|^4, |c|^2
+    MODE_ENERGY = 6, // partial sums of Re(conj(c) T c), V|c|^2, |c|^4, |c|^2
+    // the paper's own imaginary-time iteration, ca = dt/2:
+    MODE_PREP = 7,   // pointwise: psi = scale * c; out1 = psi exp(-V ca) (1 - g ca |psi|^2)       (Eq. 7, lazy scale)
+    MODE_KIN = 8,    // out1 = c - ca T c                                                          (first Euler half step)
+    MODE_SPLITB = 9  // u = c - ca T c; out1 = u exp(-V ca) (1 - g ca |u|^2); partial sum of |out1|^2
 };
 constexpr int NACC = 4;           // accumulators per block in the partial-sum array
 constexpr int STAGE_THREADS = 32;

@@ -235,7 +235,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
         }
     }
     double sc = 1.0, gsc = p.g;
-    if (MODE == MODE_IMAG) { sc = *p.scale_in; gsc = p.g * (sc * sc); }
+    if (MODE == MODE_IMAG || MODE == MODE_PREP) { sc = *p.scale_in; gsc = p.g * (sc * sc); }
 
     int niter = ne;
     if (SPW == 2) niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16));   // both halves run the same loop
@@ -255,7 +255,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     cp_async_zfill(dst + (unsigned)e * ROW_BYTES, in + (bc + (unsigned)__popc(word & bm[e])), on);
                 }
             }
-            if (i >= R && i < ne - R) {
+            if (MODE != MODE_PREP && i >= R && i < ne - R) {
                 const unsigned ti = (unsigned)((1 + hq) * G::NE + i);
                 const uint2 m = lds_u2(smask + ti * 8u);
                 const unsigned b = lds_u1(sbase + ti * 4u);
@@ -327,7 +327,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
         // ---- V(r,t) of plane c: depends on coordinates only, so its dependency chains (one per patch point,
         //      interleaved) are issued here and overlap the shared-memory latency of psi(k) --------------------
         double vpot[PR];
-        if (cany) {
+        if (cany && MODE != MODE_KIN) {
             const double zc = ((double)(kstart + ic) - p.zc) * p.pot.h + p.pot.cz;
             const double qz = p.haz * (zc * zc) - p.delta_eff;
 #pragma unroll
@@ -368,6 +368,25 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     acc[1] += vpot[e] * (double)a2;
                     acc[2] += (double)a2 * (double)a2;
                     acc[3] += (double)a2;
+                    continue;
+                }
+                if (MODE == MODE_PREP || MODE == MODE_KIN || MODE == MODE_SPLITB) {
+                    // the paper's split iteration: Euler half step of the kinetic part and / or the diagonal
+                    // propagator exp(-V ca) (1 - g ca |u|^2) of Eq. 7 with the linearised interaction factor
+                    const T ca = (T)p.ca;
+                    C u = cv;
+                    if (MODE != MODE_PREP) u = mk<T>(fma(-ca, tc.x, cv.x), fma(-ca, tc.y, cv.y));
+                    C o = u;
+                    if (MODE != MODE_KIN) {
+                        const double u2 = (double)u.x * (double)u.x + (double)u.y * (double)u.y;
+                        const T f = (T)(sc * exp(-vpot[e] * p.ca) * fma(-gsc * p.ca, u2, 1.0));
+                        o = mk<T>(u.x * f, u.y * f);
+                    }
+                    if (MODE == MODE_SPLITB) {
+                        const double o2 = (double)o.x * (double)o.x + (double)o.y * (double)o.y;
+                        acc[0] += on ? o2 : 0.0;
+                    }
+                    if (on) reinterpret_cast<C*>(p.out1)[pos] = o;
                     continue;
                 }
                 const T diag = (T)fma(gsc, (double)a2, vpot[e]);
@@ -417,7 +436,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
             PO[e] = v[e];
         }
         // ---- in-plane part (only planes of the stream itself are ever finished) ----------------------------------
-        if (i >= R && i < ne - R) {
+        if (MODE != MODE_PREP && i >= R && i < ne - R) {
             // x direction: source rows r = -R .. PR-1+R of column ly; rows 0..PR-1 are the patch itself
 #pragma unroll
             for (int r = -R; r <= PR - 1 + R; ++r) {
@@ -466,7 +485,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
     cp_async_wait<0>();
 
     // ---- per-stream partial sums in a fixed order (bit-reproducible, independent of scheduling) -------
-    if (MODE == MODE_IMAG || MODE == MODE_ENERGY) {
+    if (MODE == MODE_IMAG || MODE == MODE_ENERGY || MODE == MODE_SPLITB) {
 #pragma unroll
         for (int kq = 0; kq < NACC; ++kq)
 #pragma unroll
@@ -504,6 +523,9 @@ cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
         case MODE_S4: return launch_one<T, R, MODE_S4>(p, st);
         case MODE_IMAG: return launch_one<T, R, MODE_IMAG>(p, st);
         case MODE_ENERGY: return launch_one<T, R, MODE_ENERGY>(p, st);
+        case MODE_PREP: return launch_one<T, R, MODE_PREP>(p, st);
+        case MODE_KIN: return launch_one<T, R, MODE_KIN>(p, st);
+        case MODE_SPLITB: return launch_one<T, R, MODE_SPLITB>(p, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -523,6 +545,9 @@ cudaError_t set_attr_modes() {
     if ((e = set_attr<T, R, MODE_S4>())) return e;
     if ((e = set_attr<T, R, MODE_IMAG>())) return e;
     if ((e = set_attr<T, R, MODE_ENERGY>())) return e;
+    if ((e = set_attr<T, R, MODE_PREP>())) return e;
+    if ((e = set_attr<T, R, MODE_KIN>())) return e;
+    if ((e = set_attr<T, R, MODE_SPLITB>())) return e;
     return cudaSuccess;
 }
 

@@ -162,3 +162,20 @@ def test_config2_full_imaginary_time(P):
         if e_prev is not None:
             assert e["total"] < e_prev                    # imaginary time lowers the energy (invariant)
         e_prev = e["total"]
+
+
+def test_config2_split_scheme_iterations(P):
+    """BASELINE configs[1] with the paper's own iteration: 10 iterations on the whole grid
+    against the NumPy oracle (imag_split_step)."""
+    from oracle import gpe_oracle as O
+    w = I.config2()
+    box, pot, act = oracle_objs(w)
+    grid = P.Grid.from_workload(w)
+    sim = P.Sim(grid, "complex128", w.stencil, w.g)
+    og = O.SparseGrid(box, act, RADIUS[w.stencil])
+    psi = I.make_psi0(w, act)
+    sim.set_psi_host(psi)
+    sim.run_imag_split(w.dt, 10)
+    ref = O.run_imag_split(og, pot, w.g, 0.0, w.dt, 10, psi, w.stencil)
+    assert rel_max(sim.get_psi_host(), ref) < 1e-11
+    assert abs(sim.norm() - 1.0) < 1e-12

@@ -167,3 +167,24 @@ def test_config1_complex64_1000_steps(P):
     sim.run_rk4(w.dt, 1000)
     ref = co.run_rk4(w.g, 0.0, w.dt, 1000, psi.astype(np.complex128))
     assert rel_max(sim.get_psi_host(), ref) < 1e-3
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_imag_split_small_shell(P, stencil, dtype):
+    """The paper's own ground-state iteration (Eq. 7 half steps with the linearised interaction
+    factor, two forward-Euler kinetic half steps, renormalisation) against the oracle's imag_split_step."""
+    w = I.small_shell(40, stencil, dtype).with_(g=400.0)
+    box, pot, act, grid, sim = _make(P, w)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    sim.run_imag_split(2e-3, 7)
+    sim.imag_split_step(2e-3)
+    ref = O.run_imag_split(og, pot, w.g, 0.0, 2e-3, 8, psi.astype(np.complex128), stencil)
+    assert rel_max(sim.get_psi_host(), ref) < (1e-12 if dtype == "complex128" else 1e-5)
+    assert abs(sim.norm() - 1.0) < (1e-12 if dtype == "complex128" else 1e-5)
+    if dtype == "complex128":
+        # both schemes lower the energy from the same start, and the Euler scheme follows within O(dt)
+        e0 = O.energy(og, pot, w.g, 0.0, psi.astype(np.complex128), stencil)["total"]
+        assert sim.energy()["total"] < e0

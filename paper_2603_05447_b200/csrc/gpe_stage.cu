@@ -99,9 +99,12 @@ __device__ __forceinline__ double fast_sqrt(double s) {
 }
 
 constexpr int KZMAX = 32;                 // planes per stream (host splits work items to at most this)
-constexpr int PF = 2;                     // planes in flight per stream (cp.async groups)
-constexpr int NSLOT = PF + 1;             // ring of plane slots per stream
-constexpr int NAUX = PF + 1;              // ring of aux-plane slots per stream
+// planes in flight per stream (cp.async groups): the 7-point kernels are bound by global-load latency (84
+// registers, small slots: three planes ahead), the 13-point ones by the shared-memory pipe (two)
+#ifndef GPE_PF_R1
+#define GPE_PF_R1 3
+#endif
+__host__ __device__ constexpr int pf_of(int radius) { return radius == 1 ? GPE_PF_R1 : 3; }
 constexpr int STAGE_WARPS = STAGE_THREADS / 32;
 
 // Shared memory of one stream.  Plane slot: (8+2R) rows (x) of PY values, the tile at rows/cols R..R+7 and
@@ -113,6 +116,8 @@ template <typename T, int R, bool AUX> struct Geo {
     static constexpr int PY = (sizeof(T) == 4 && R == 2) ? 14 : 8 + 2 * R;
     static constexpr int PLANE = ROWS * PY;                 // values per slot
     static constexpr int NE = KZMAX + 2 * R;                // table entries per tile
+    static constexpr int NSLOT = pf_of(R) + 1;              // ring of plane slots per stream
+    static constexpr int NAUX = pf_of(R) + 1;               // ring of aux-plane slots per stream
     static constexpr int RING_BYTES = NSLOT * PLANE * ES;
     static constexpr int AUX_BYTES = AUX ? NAUX * 64 * ES : 0;
     static constexpr int MASK_OFF = RING_BYTES + AUX_BYTES;  // [5][NE] (lo, hi)
@@ -137,6 +142,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
     using C = typename CxOf<T>::type;
     constexpr bool HAS_AUX = mode_has_aux(MODE);
     using G = Geo<T, R, HAS_AUX>;
+    constexpr int PF = pf_of(R), NSLOT = G::NSLOT, NAUX = G::NAUX;
     constexpr unsigned ES = G::ES;
     constexpr int LPS = 64 / PR;                           // lanes per stream (16: half-warp, 32: warp)
     constexpr int SPW = 32 / LPS;                          // streams per warp

@@ -58,7 +58,7 @@ struct Slab {                // one z-plane of one tile
     long long base;          // storage position of the slab's first lane
 };
 
-// One stream (half-warp's worth of work): nz consecutive planes of one tile (a piece of a work item).
+// One stream (a warp's worth of work): nz consecutive planes of one tile (a piece of a work item).
 // eoff[q] + zp = slab entry of plane zp in tile q (0 = own, 1..4 = -x,+x,-y,+y), valid for
 // zlo[q] <= zp < zhi[q] (zlo = zhi = 0 when the neighbour tile is absent).
 struct alignas(16) WorkRec {

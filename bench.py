@@ -362,6 +362,64 @@ def run_ours(args, w):
     print(json.dumps(line), flush=True)
 
 
+SWEEP_TARGETS = (9.5e4, 3e5, 1e6, 3e6, 1e7, 3e7, 1e8, 3e8)
+
+
+def run_sweep(args):
+    """BASELINE configs[4]: isotropic dressed shells of fixed thickness (24 points) from 1e5 to 3e8 active points
+    (boxes 64^3 to 2048^3), 7- and 13-point stencils, complex64 and complex128, 50 RK4 steps each, plus the
+    fully active 512^3 box.  One JSON line per point (device-resident timing only; the state is a uniform
+    amplitude with seeded phase noise drawn by the device generator: throughput does not depend on it)."""
+    import torch
+    import paper_2603_05447_b200 as P
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, peak_src = measured_peak()
+    targets = [t for t in SWEEP_TARGETS if t <= args.sweep_max]
+    points = [("shell", t) for t in targets] + [("dense", 512)]
+    for kind, t in points:
+        w0 = I.config5_shell(t, 24, 13, "complex128", 0) if kind == "shell" else I.config5_dense(512, 13, "complex128")
+        grid = P.Grid.from_workload(w0)
+        n = grid.n_active
+        for stencil in (7, 13):
+            for dtype in ("complex128", "complex64"):
+                w = (I.config5_shell(t, 24, stencil, dtype, 0) if kind == "shell" else I.config5_dense(512, stencil, dtype))
+                sim = P.Sim(grid, dtype, stencil, w.g, device="cuda:0")
+                gen = torch.Generator(device=dev)
+                gen.manual_seed(w.seed)
+                ph = 1e-3 * (2.0 * torch.rand(n, device=dev, dtype=torch.float64, generator=gen) - 1.0)
+                psi = torch.polar(torch.full((n,), (1.0 / (n * w.h ** 3)) ** 0.5, device=dev, dtype=torch.float64), ph)
+                sim.set_psi(psi.to(sim.cdtype))
+                del psi, ph
+                sim.time = 0.0
+                for _ in range(max(args.warmup, 3)):
+                    sim.run_rk4(w.dt, 1)
+                torch.cuda.synchronize(dev)
+                stream = torch.cuda.current_stream()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                steps = 50
+                e0.record(stream)
+                sim.run_rk4(w.dt, steps)
+                e1.record(stream)
+                torch.cuda.synchronize(dev)
+                ms = e0.elapsed_time(e1)
+                nrm = sim.norm()
+                csize = 16 if dtype == "complex128" else 8
+                value = stage_updates_per_s(float(n), steps, ms)
+                gbps = value * 3 * csize / 1e9
+                print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": steps,
+                                  "ms_per_step": ms / steps, "dtype": "c128" if dtype == "complex128" else "c64",
+                                  "data": "synthetic", "config": {"workload": w.name, "box": [w.nx, w.ny, w.nz],
+                                                                   "stencil": stencil, "n_active": n,
+                                                                   "active_fraction": n / (w.nx * w.ny * w.nz)},
+                                  "hbm_GBps_algorithmic": gbps, "frac_of_measured_peak": gbps / peak,
+                                  "peak": peak, "norm_after": nrm}), flush=True)
+                sim.close()
+                del sim
+                torch.cuda.empty_cache()
+        grid.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -371,8 +429,12 @@ def main():
     ap.add_argument("--workload", default="cfg4_c128", choices=sorted(workloads()))
     ap.add_argument("--kz", type=int, default=0, help="planes per thread block (0 = library default)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE configs[4] bandwidth sweep: one JSON line per point")
+    ap.add_argument("--sweep-max", type=float, default=3e8, help="largest target point count of the sweep")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.sweep:
+        return run_sweep(args)
     w = workloads()[args.workload]
     if args.impl == "reference":
         run_reference(args, w)

@@ -184,6 +184,15 @@ int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 int gpe_imag_step(gpe_sim* s, double dt, void* stream);
 int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 
+/* Re-gridding between ramp stages ("the grid post-selection procedure is repeated, and the
+ * wavefunction is remapped between the old and new grids").  dst's state becomes src's
+ * state on the points the two active sets share and 0 on the points that are new; values on points that are
+ * dropped are lost (the caller checks gpe_norm(dst) and picks the cutoff, e.g. the paper's 5 max(mu_i, mu_i+1)).
+ * Both sims must have the same precision and grids post-selected from the same bounding box (nx, ny, nz, h,
+ * center), else INVALID_ARG.  dst's clock is set to src's.  The index match is one merge pass on the host over
+ * the two ascending index lists; the values move on the device (unpack, gather, pack).  Synchronises `stream`. */
+int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream);
+
 /* a5 (second mode): the paper's own ground-state iteration, in its order (PAPER.md:60-67,
  * :87 kernels K1-K3, footnote [44] at :236), V frozen at the sim clock:
  *   psi <- psi exp(-V dt/2) (1 - g |psi|^2 dt/2)        Eq. 7 for dt/2, interaction factor linearised (:67)

@@ -287,6 +287,20 @@ def run_imag_split(grid, pot, g, t, dt, nsteps, psi, stencil, n_target=1.0):
     return psi
 
 
+def remap_psi(active_old: np.ndarray, psi_old: np.ndarray, active_new: np.ndarray) -> np.ndarray:
+    """Re-gridding between ramp stages ("the wavefunction is remapped between the old and new
+    grids"): the value of a point that is in both active sets is kept, a point that is new starts at 0 (psi = 0
+    outside the old region of interest), a point that is dropped is lost.  Explicit loop over a
+    dictionary of the old points."""
+    old = {int(L): k for k, L in enumerate(active_old)}
+    out = np.zeros(len(active_new), dtype=np.complex128)
+    for i, L in enumerate(active_new):
+        k = old.get(int(L))
+        if k is not None:
+            out[i] = psi_old[k]
+    return out
+
+
 def energy(grid, pot, g, t, psi, stencil) -> dict:
     """Discrete GP functional with the same discrete Laplacian (R8).
 

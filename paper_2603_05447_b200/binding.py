@@ -63,6 +63,7 @@ SYMBOLS = (
     "gpe_set_time", "gpe_get_time", "gpe_apply_H", "gpe_step_rk4", "gpe_run_rk4", "gpe_imag_step",
     "gpe_run_imag", "gpe_norm", "gpe_energy", "gpe_sim_kernel_launches", "gpe_sim_time_stages",
     "gpe_sim_stage_time_ms", "gpe_sim_set_planes_per_block", "gpe_imag_split_step", "gpe_run_imag_split",
+    "gpe_remap_psi",
 )
 
 _lib = None
@@ -275,6 +276,10 @@ class Sim:
 
     def run_imag_split(self, dt, nsteps, stream=None):
         _check(lib().gpe_run_imag_split(self._h, C.c_double(dt), C.c_int64(nsteps), _stream_ptr(stream)))
+
+    def remap_from(self, src: "Sim", stream=None):
+        """Re-gridding: take src's state on the shared points, 0 on the new ones."""
+        _check(lib().gpe_remap_psi(src._h, self._h, _stream_ptr(stream)))
 
     # -- reductions (synchronise the stream) ------------------------------------------------------------
     def norm(self, stream=None) -> float:

@@ -407,6 +407,42 @@ int gpe_get_psi(gpe_sim* s, void* dev_psi_canonical, void* stream) {
     return GPE_OK;
 }
 
+int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream) {
+    if (!src || !dst || src == dst) return fail(GPE_ERR_INVALID_ARG, "null or identical simulations");
+    if (src->dtype != dst->dtype) return fail(GPE_ERR_INVALID_ARG, "source and destination precisions differ");
+    const gpe_box &a = src->grid->h.box, &b = dst->grid->h.box;
+    if (a.nx != b.nx || a.ny != b.ny || a.nz != b.nz || a.h != b.h || a.center[0] != b.center[0] ||
+        a.center[1] != b.center[1] || a.center[2] != b.center[2])
+        return fail(GPE_ERR_INVALID_ARG, "the two grids must be post-selected from the same bounding box");
+    dst->t = src->t;
+    if (dst->n == 0) return GPE_OK;
+    // new canonical rank -> old canonical rank (both index lists ascend: one merge pass), -1 = new point
+    const std::vector<int64_t>&ia = src->grid->h.active_idx, &ib = dst->grid->h.active_idx;
+    std::vector<int64_t> map((size_t)dst->n);
+    size_t j = 0;
+    for (size_t i = 0; i < ib.size(); ++i) {
+        while (j < ia.size() && ia[j] < ib[i]) ++j;
+        map[i] = (j < ia.size() && ia[j] == ib[i]) ? (int64_t)j : -1;
+    }
+    int64_t* d_map = nullptr;
+    cudaError_t e = cudaMalloc(&d_map, map.size() * sizeof(int64_t));
+    if (e == cudaErrorMemoryAllocation) return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(remap table)");
+    CU(e);
+    cudaStream_t st = (cudaStream_t)stream;
+    e = cudaMemcpyAsync(d_map, map.data(), map.size() * sizeof(int64_t), cudaMemcpyHostToDevice, st);
+    int rc = 0;
+    if (e == cudaSuccess && src->n > 0) rc = launch_unpack(src->dtype, src->buf[0], src->staging, src->grid->d_perm, src->n, stream);
+    if (e == cudaSuccess && !rc) rc = launch_remap(dst->dtype, src->staging, dst->staging, d_map, dst->n, stream);
+    if (e == cudaSuccess && !rc) rc = launch_pack(dst->dtype, dst->staging, dst->buf[0], dst->grid->d_perm, dst->n, stream);
+    if (e == cudaSuccess && !rc) e = cudaStreamSynchronize(st);   // the table is freed below
+    cudaFree(d_map);
+    if (e != cudaSuccess) return cuda_fail(e, "gpe_remap_psi");
+    if (rc) return cuda_fail((cudaError_t)rc, "gpe_remap_psi kernels");
+    src->launches += src->n > 0 ? 1 : 0;
+    dst->launches += 2;
+    return GPE_OK;
+}
+
 int gpe_set_psi_host(gpe_sim* s, const void* host_psi_canonical, void* stream) {
     if (!s || (!host_psi_canonical && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
     if (s->n == 0) return GPE_OK;

@@ -128,6 +128,8 @@ size_t stage_smem_bytes(int dtype, int radius);
 int stage_max_planes();   // upper bound of WorkRec::nz the stage kernels accept
 int launch_pack(int dtype, const void* canonical, void* storage, const int64_t* perm, int64_t n, void* stream);
 int launch_unpack(int dtype, const void* storage, void* canonical, const int64_t* perm, int64_t n, void* stream);
+// dst_canonical[i] = map[i] >= 0 ? src_canonical[map[i]] : 0   (re-gridding)
+int launch_remap(int dtype, const void* src_canonical, void* dst_canonical, const int64_t* map, int64_t n_dst, void* stream);
 // partials[b*NACC + 0] = sum over the block's contiguous chunk of |psi|^2; nblk = norm_blocks(n)
 int norm_blocks(int64_t n);
 int launch_norm_partials(int dtype, const void* storage, int64_t n, double* partials, void* stream);

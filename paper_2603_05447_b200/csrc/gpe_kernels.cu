@@ -28,6 +28,18 @@ __global__ void unpack_kernel(const C* __restrict__ storage, C* __restrict__ can
         canonical[perm[s]] = storage[s];
 }
 
+// re-gridding: dst[i] = src[map[i]] or 0 where the new point was not in the old grid (canonical order)
+template <typename C>
+__global__ void remap_kernel(const C* __restrict__ src, C* __restrict__ dst, const int64_t* __restrict__ map, int64_t n) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t m = map[i];
+        C v;
+        v.x = 0; v.y = 0;
+        if (m >= 0) v = src[m];
+        dst[i] = v;
+    }
+}
+
 constexpr int NORM_THREADS = 256;
 constexpr int NORM_CHUNK = 8192;   // elements per block
 constexpr int NORM_MAX_BLOCKS = 148 * 16;
@@ -118,6 +130,16 @@ int launch_unpack(int dtype, const void* storage, void* canonical, const int64_t
         unpack_kernel<double2><<<grid_for(n, 256), 256, 0, st>>>((const double2*)storage, (double2*)canonical, perm, n);
     else
         unpack_kernel<float2><<<grid_for(n, 256), 256, 0, st>>>((const float2*)storage, (float2*)canonical, perm, n);
+    return (int)cudaGetLastError();
+}
+
+int launch_remap(int dtype, const void* src_canonical, void* dst_canonical, const int64_t* map, int64_t n_dst, void* stream) {
+    if (n_dst <= 0) return 0;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == GPE_C128)
+        remap_kernel<double2><<<grid_for(n_dst, 256), 256, 0, st>>>((const double2*)src_canonical, (double2*)dst_canonical, map, n_dst);
+    else
+        remap_kernel<float2><<<grid_for(n_dst, 256), 256, 0, st>>>((const float2*)src_canonical, (float2*)dst_canonical, map, n_dst);
     return (int)cudaGetLastError();
 }
 

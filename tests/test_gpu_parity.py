@@ -188,3 +188,29 @@ def test_imag_split_small_shell(P, stencil, dtype):
         # both schemes lower the energy from the same start, and the Euler scheme follows within O(dt)
         e0 = O.energy(og, pot, w.g, 0.0, psi.astype(np.complex128), stencil)["total"]
         assert sim.energy()["total"] < e0
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+def test_regrid_remap(P, dtype):
+    """Re-gridding between ramp stages: the state is carried from the shell at Delta = 14 to the
+    post-selection at Delta = 22 (a larger, partly overlapping shell) and evolved on; against the oracle."""
+    wa = I.small_shell(40, 13, dtype).with_(delta0=14.0, delta1=14.0)
+    wb = wa.with_(delta0=22.0, delta1=22.0)
+    box, pot_a, act_a, grid_a, sim_a = _make(P, wa)
+    _, pot_b, act_b, grid_b, sim_b = _make(P, wb)
+    assert 0 < np.intersect1d(act_a, act_b).size < min(act_a.size, act_b.size)
+    psi = I.make_psi0(wa, act_a).astype(sim_a.npdtype)
+    sim_a.set_psi_host(psi)
+    sim_a.time = 0.25
+    sim_b.remap_from(sim_a)
+    want = O.remap_psi(act_a, psi.astype(np.complex128), act_b)
+    assert np.array_equal(sim_b.get_psi_host(), want.astype(sim_b.npdtype))     # a copy: bit-exact
+    assert sim_b.time == 0.25
+    sim_b.run_rk4(wb.dt, 2)
+    og = O.SparseGrid(box, act_b, 2)
+    ref = O.run_rk4(og, pot_b, wb.g, 0.25, wb.dt, 2, want, 13)
+    assert rel_max(sim_b.get_psi_host(), ref) < (1e-12 if dtype == "complex128" else 1e-5)
+    # different precision or box: refused
+    other = P.Sim(grid_b, "complex64" if dtype == "complex128" else "complex128", 13, wb.g)
+    with pytest.raises(P.GpeError):
+        other.remap_from(sim_a)

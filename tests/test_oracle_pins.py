@@ -522,3 +522,24 @@ def test_P13_linearised_interaction_factor():
     ratio = lin / exact                                        # = (1 - x) e^{x} = 1 - x^2/2 - x^3/3 - ...
     assert np.max(np.abs(ratio - (1 - x) * np.exp(x))) < 1e-14
     assert np.all(ratio.real <= 1.0) and np.max(np.abs(1 - ratio.real - x ** 2 / 2)) < x.max() ** 3
+
+
+# ---- P14: re-gridding -----------------------------------------------------------------------
+def test_P14_remap_is_restriction_and_zero_extension():
+    """What the remap is fixed by: on a dense array it is "scatter the old values into the box, read the new
+    points" (zero where nothing was scattered); shared points keep their value, round trips lose exactly the
+    points that were dropped, and the norm splits into kept + dropped."""
+    nx, ny, nz = 7, 6, 9
+    a = I.random_mask_lin(21, nx, ny, nz, 0.5)
+    b = I.random_mask_lin(22, nx, ny, nz, 0.6)
+    psi = I.random_psi(23, a.size)
+    dense = np.zeros(nx * ny * nz, np.complex128)
+    dense[a] = psi
+    got = O.remap_psi(a, psi, b)
+    assert np.array_equal(got, dense[b])
+    back = O.remap_psi(b, got, a)
+    shared = np.isin(a, b)
+    assert np.array_equal(back[shared], psi[shared]) and np.all(back[~shared] == 0)
+    assert abs(np.sum(np.abs(got) ** 2) + np.sum(np.abs(psi[~shared]) ** 2) - np.sum(np.abs(psi) ** 2)) < 1e-12
+    assert O.remap_psi(a, psi, np.zeros(0, np.int64)).size == 0
+    assert np.all(O.remap_psi(np.zeros(0, np.int64), np.zeros(0, np.complex128), b) == 0)

@@ -176,6 +176,13 @@ int gpe_apply_H(gpe_sim* s, double t, const void* dev_in_canonical, void* dev_ou
 int gpe_step_rk4(gpe_sim* s, double dt, void* stream);
 int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 
+/* The paper's cheaper integrator: Heun's third-order method "RKHE3" in the
+ * stage-state form of Eq. A6-A7 with a* = [[1,0],[1,0]], b* = [1/4, 3/4, 0] (PAPER.md:286-290 Eq. A8-A9): three
+ * fused stage kernels per step, y2 = y0 + dt/3 f(t, y0); y3 = y0 + 2dt/3 f(t + dt/3, y2) and p = y0/4 + 3 y2/4;
+ * y_new = p + 3dt/4 f(t + 2dt/3, y3).  9 complex values per point and step (RK4: 12).  Clock as gpe_run_rk4. */
+int gpe_step_rkhe3(gpe_sim* s, double dt, void* stream);
+int gpe_run_rkhe3(gpe_sim* s, double dt, int64_t nsteps, void* stream);
+
 /* a5: psi' = psi - dt H[psi] psi, psi <- psi' sqrt(n_target / (h^3 sum|psi'|^2)) with V frozen at the sim
  * clock (PAPER.md:35, :60 Eq. 6, :87; forward-Euler reading DESIGN.md R7).  One fused kernel per step
  * (update + block partial sums) + a one-block finalise; the scale is applied lazily at the next load as

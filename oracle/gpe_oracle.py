@@ -235,6 +235,24 @@ def run_rk4(grid, pot, g, t0, dt, nsteps, psi, stencil):
     return psi
 
 
+def rkhe3_step(grid, pot, g, t, dt, psi, stencil):
+    """Heun's third-order method ("RKHE3") on d psi/dt = -i H psi, textbook k form:
+    c = (0, 1/3, 2/3), a21 = 1/3, a32 = 2/3, b = (1/4, 0, 3/4).  The product uses the paper's memory-optimised
+    form (PAPER.md:286-290 Eq. A8-A9: a* = [[1,0],[1,0]], b* = [1/4, 3/4, 0])."""
+    def f(tt, y):
+        return -1j * apply_H(grid, pot, g, tt, y, stencil)
+    k1 = f(t, psi)
+    k2 = f(t + dt / 3.0, psi + (dt / 3.0) * k1)
+    k3 = f(t + 2.0 * dt / 3.0, psi + (2.0 * dt / 3.0) * k2)
+    return psi + dt * (0.25 * k1 + 0.75 * k3)
+
+
+def run_rkhe3(grid, pot, g, t0, dt, nsteps, psi, stencil):
+    for n in range(nsteps):
+        psi = rkhe3_step(grid, pot, g, t0 + n * dt, dt, psi, stencil)
+    return psi
+
+
 def _sum(x) -> float:
     return float(np.sum(np.asarray(x, dtype=np.longdouble)))
 

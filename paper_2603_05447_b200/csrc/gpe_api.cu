@@ -185,12 +185,14 @@ StageParams base_params(const gpe_sim* s, double t) {
     p.hax = 0.5 * h.pot.ax; p.hay = 0.5 * h.pot.ay; p.haz = 0.5 * h.pot.az;
     p.om2 = h.pot.omega * h.pot.omega;
     p.delta_eff = h.pot.kind == GPE_POT_DRESSED ? p.pot.delta : 0.0;
+    p.comb[0] = -1.0 / 3.0; p.comb[1] = 1.0 / 3.0; p.comb[2] = 2.0 / 3.0;   // RK4 b* (Eq. A11)
     return p;
 }
 
 int stage(gpe_sim* s, int mode, double t, double ca, const void* in, const void* aux, void* out1, void* out2,
-          void* stream, int timed_slot = -1) {
+          void* stream, int timed_slot = -1, const double* comb = nullptr) {
     StageParams p = base_params(s, t);
+    if (comb) { p.comb[0] = comb[0]; p.comb[1] = comb[1]; p.comb[2] = comb[2]; }
     p.ca = ca; p.in = in; p.aux = aux; p.out1 = out1; p.out2 = out2;
     cudaStream_t st = (cudaStream_t)stream;
     if (s->timing && timed_slot >= 0) {
@@ -220,6 +222,18 @@ int rk4_step(gpe_sim* s, double t, double dt, void* stream) {
     if ((rc = stage(s, MODE_S2, t + 0.5 * dt, 0.5 * dt, B, A, C, D, stream, 1))) return rc;             // y3, p
     if ((rc = stage(s, MODE_S3, t + 0.5 * dt, dt, C, A, B, nullptr, stream, 2))) return rc;             // y4
     if ((rc = stage(s, MODE_S4, t + dt, dt / 6.0, B, D, A, nullptr, stream, 3))) return rc;             // y_new
+    return GPE_OK;
+}
+
+int rkhe3_step(gpe_sim* s, double t, double dt, void* stream) {
+    void *A = s->buf[0], *B = s->buf[1], *C = s->buf[2], *D = s->buf[3];
+    int rc;
+    // Heun's third-order method, PAPER.md:276-281 Eq. A6-A7 with a* = [[1,0],[1,0]], b* = [1/4, 3/4, 0] (Eq. A8-A9)
+    // and a21 = 1/3, a32 = 2/3, b3 = 3/4; the b* terms are pre-summed into p by the second stage
+    const double comb[3] = {0.25, 0.75, 0.0};
+    if ((rc = stage(s, MODE_S1, t, dt / 3.0, A, nullptr, B, nullptr, stream))) return rc;                           // y2
+    if ((rc = stage(s, MODE_S2, t + dt / 3.0, 2.0 * dt / 3.0, B, A, C, D, stream, -1, comb))) return rc;            // y3, p
+    if ((rc = stage(s, MODE_S3, t + 2.0 * dt / 3.0, 0.75 * dt, C, D, A, nullptr, stream))) return rc;               // y_new
     return GPE_OK;
 }
 
@@ -506,6 +520,20 @@ int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
 }
 
 int gpe_step_rk4(gpe_sim* s, double dt, void* stream) { return gpe_run_rk4(s, dt, 1, stream); }
+
+int gpe_run_rkhe3(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
+    const double t0 = s->t;
+    for (int64_t n = 0; n < nsteps; ++n) {
+        int rc = rkhe3_step(s, t0 + (double)n * dt, dt, stream);
+        if (rc) return rc;
+    }
+    s->t = t0 + (double)nsteps * dt;
+    return GPE_OK;
+}
+
+int gpe_step_rkhe3(gpe_sim* s, double dt, void* stream) { return gpe_run_rkhe3(s, dt, 1, stream); }
 
 int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");

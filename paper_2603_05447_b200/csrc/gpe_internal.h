@@ -85,7 +85,7 @@ struct PotDev {
 enum Mode : int {
     MODE_APPLY = 0,  // out1 = H c
     MODE_S1 = 1,     // out1 = c + ca * f(c)                        f(c) = -i H c
-    MODE_S2 = 2,     // out1 = aux + ca * f(c); out2 = -1/3 aux + 1/3 c + 2/3 out1
+    MODE_S2 = 2,     // out1 = aux + ca * f(c); out2 = comb[0] aux + comb[1] c + comb[2] out1  (RK4: -1/3, 1/3, 2/3)
     MODE_S3 = 3,     // out1 = aux + ca * f(c)
     MODE_S4 = 4,     // out1 = aux + 1/3 c + ca * f(c)
     MODE_IMAG = 5,   // psi = scale * c; out1 = psi - ca * H psi; partial sum of |out1|^2
@@ -114,6 +114,7 @@ struct StageParams {
     double hax, hay, haz;  // 0.5 a_x, 0.5 a_y, 0.5 a_z
     double om2;            // Omega^2
     double delta_eff;      // Delta(t) for the dressed potential, 0 for the harmonic one
+    double comb[3];        // MODE_S2: out2 = comb[0] aux + comb[1] c + comb[2] out1 (the b* terms known so far, Eq. A7)
     const void* in;        // array the stencil is applied to (storage order)
     const void* aux;       // y0 or p (storage order) or null
     void* out1;

@@ -416,8 +416,8 @@ stage_kernel(const __grid_constant__ StageParams p) {
                         o.y = fma(third, cv.y, o.y);
                     }
                     if (MODE == MODE_S2) {
-                        const T third = (T)(1.0 / 3.0), tt = (T)(2.0 / 3.0);
-                        const C o2 = mk<T>(fma(tt, o.x, third * (cv.x - av[e].x)), fma(tt, o.y, third * (cv.y - av[e].y)));
+                        const T b0 = (T)p.comb[0], b1 = (T)p.comb[1], b2 = (T)p.comb[2];
+                        const C o2 = mk<T>(fma(b2, o.x, fma(b1, cv.x, b0 * av[e].x)), fma(b2, o.y, fma(b1, cv.y, b0 * av[e].y)));
                         if (on) reinterpret_cast<C*>(p.out2)[pos] = o2;
                     }
                 }

@@ -214,3 +214,21 @@ def test_regrid_remap(P, dtype):
     other = P.Sim(grid_b, "complex64" if dtype == "complex128" else "complex128", 13, wb.g)
     with pytest.raises(P.GpeError):
         other.remap_from(sim_a)
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_rkhe3_small_shell_with_ramp(P, stencil, dtype):
+    """Heun's third-order method in the paper's stage-state form (PAPER.md Eq. A6-A9) against the textbook
+    k1..k3 oracle, time-ramped potential (stage times t, t + dt/3, t + 2dt/3)."""
+    w = I.small_shell(40, stencil, dtype).with_(delta0=14.0, delta1=22.0, t_ramp=0.02)
+    box, pot, act, grid, sim = _make(P, w)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    sim.time = 0.005
+    sim.run_rkhe3(w.dt, 4)
+    sim.step_rkhe3(w.dt)
+    assert abs(sim.time - (0.005 + 5 * w.dt)) < 1e-15
+    ref = O.run_rkhe3(og, pot, w.g, 0.005, w.dt, 5, psi.astype(np.complex128), stencil)
+    assert rel_max(sim.get_psi_host(), ref) < (1e-12 if dtype == "complex128" else 1e-5)

@@ -543,3 +543,45 @@ def test_P14_remap_is_restriction_and_zero_extension():
     assert abs(np.sum(np.abs(got) ** 2) + np.sum(np.abs(psi[~shared]) ** 2) - np.sum(np.abs(psi) ** 2)) < 1e-12
     assert O.remap_psi(a, psi, np.zeros(0, np.int64)).size == 0
     assert np.all(O.remap_psi(np.zeros(0, np.int64), np.zeros(0, np.complex128), b) == 0)
+
+
+# ---- P15: Heun's third-order method (RKHE3, A8-A9) ------------------------------------------------
+def test_P15_rkhe3_amplification_factor_and_stage_form():
+    """g = 0, static V: on an eigenvector of H one step multiplies by R(z) = 1 + z + z^2/2 + z^3/6, z = -i E dt
+    (any third-order three-stage method); and the paper's stage-state form (Eq. A6-A9) gives the same step."""
+    n, h = 12, 0.6
+    box, grid = full_box_grid(n, n, n, h)
+    pot = O.Potential(kind=O.HARMONIC)
+    e1, v1 = ho_ground_state_1d(n, h, 7)
+    psi = (v1[:, None, None] * v1[None, :, None] * v1[None, None, :]).ravel().astype(np.complex128)
+    dt = 0.05
+    z = -1j * 3 * e1 * dt
+    got = O.rkhe3_step(grid, pot, 0.0, 0.0, dt, psi, 7)
+    assert np.max(np.abs(got - (1 + z + z * z / 2 + z ** 3 / 6) * psi)) < 1e-13
+    # stage-state form with a ramped potential and g > 0 (stage times t, t + dt/3, t + 2dt/3)
+    w = I.small_shell(20, 13)
+    box = O.Box(w.nx, w.ny, w.nz, w.h)
+    pot = O.Potential(w.kind, w.ax, w.ay, w.az, 5.0, 20.0, 0.01, w.omega)
+    act = O.active_indices(box, pot, w.v_cut, O.MASK_UNION)
+    grid = O.SparseGrid(box, act, 2)
+    y0 = I.make_psi0(w, act)
+    t, dt, g = 0.003, 1e-3, w.g
+    f = lambda tt, y: -1j * O.apply_H(grid, pot, g, tt, y, 13)
+    y2 = y0 + dt / 3 * f(t, y0)                               # a* row 1: [1]
+    y3 = y0 + 2 * dt / 3 * f(t + dt / 3, y2)                  # a* row 2: [1, 0]
+    ynew = y0 / 4 + 3 * y2 / 4 + 3 * dt / 4 * f(t + 2 * dt / 3, y3)   # b* = [1/4, 3/4, 0], b_3 = 3/4
+    ref = O.rkhe3_step(grid, pot, g, t, dt, y0, 13)
+    assert np.max(np.abs(ynew - ref)) < 1e-14 * np.max(np.abs(ref))
+
+
+def test_P15_rkhe3_is_third_order():
+    w = I.small_shell(20, 7)
+    box = O.Box(w.nx, w.ny, w.nz, w.h)
+    pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
+    act = O.active_indices(box, pot, w.v_cut, w.mask_mode)
+    grid = O.SparseGrid(box, act, 1)
+    y0 = I.make_psi0(w, act)
+    T = 0.02
+    ref = O.run_rk4(grid, pot, w.g, 0.0, T / 64, 64, y0, 7)
+    errs = [np.max(np.abs(O.run_rkhe3(grid, pot, w.g, 0.0, T / n, n, y0, 7) - ref)) for n in (4, 8, 16)]
+    assert 6.5 < errs[0] / errs[1] < 9.5 and 6.5 < errs[1] / errs[2] < 9.5

@@ -253,6 +253,41 @@ def run_rkhe3(grid, pot, g, t0, dt, nsteps, psi, stencil):
     return psi
 
 
+# Cash-Karp tableau ("RKCK"; J. R. Cash and A. H. Karp 1990), fifth-order weights.
+RKCK_C = (0.0, 1.0 / 5.0, 3.0 / 10.0, 3.0 / 5.0, 1.0, 7.0 / 8.0)
+RKCK_A = ((),
+          (1.0 / 5.0,),
+          (3.0 / 40.0, 9.0 / 40.0),
+          (3.0 / 10.0, -9.0 / 10.0, 6.0 / 5.0),
+          (-11.0 / 54.0, 5.0 / 2.0, -70.0 / 27.0, 35.0 / 27.0),
+          (1631.0 / 55296.0, 175.0 / 512.0, 575.0 / 13824.0, 44275.0 / 110592.0, 253.0 / 4096.0))
+RKCK_B = (37.0 / 378.0, 0.0, 250.0 / 621.0, 125.0 / 594.0, 0.0, 512.0 / 1771.0)
+
+
+def rkck_step(grid, pot, g, t, dt, psi, stencil):
+    """One step of the Cash-Karp method (fifth-order solution) on d psi/dt = -i H psi, textbook k form
+    (PAPER.md:248-252 Eq. A1: y^(i) = y0 + dt sum_{j<i} a_ij k_j).  The product uses the paper's memory-optimised
+    form with a*, b* of PAPER.md:321-329 Eq. A12-A13."""
+    def f(tt, y):
+        return -1j * apply_H(grid, pot, g, tt, y, stencil)
+    k = []
+    for i in range(6):
+        y = psi
+        for j in range(i):
+            y = y + (dt * RKCK_A[i][j]) * k[j]
+        k.append(f(t + RKCK_C[i] * dt, y))
+    out = psi
+    for i in range(6):
+        out = out + (dt * RKCK_B[i]) * k[i]
+    return out
+
+
+def run_rkck(grid, pot, g, t0, dt, nsteps, psi, stencil):
+    for n in range(nsteps):
+        psi = rkck_step(grid, pot, g, t0 + n * dt, dt, psi, stencil)
+    return psi
+
+
 def _sum(x) -> float:
     return float(np.sum(np.asarray(x, dtype=np.longdouble)))
 

@@ -585,3 +585,70 @@ def test_P15_rkhe3_is_third_order():
     ref = O.run_rk4(grid, pot, w.g, 0.0, T / 64, 64, y0, 7)
     errs = [np.max(np.abs(O.run_rkhe3(grid, pot, w.g, 0.0, T / n, n, y0, 7) - ref)) for n in (4, 8, 16)]
     assert 6.5 < errs[0] / errs[1] < 9.5 and 6.5 < errs[1] / errs[2] < 9.5
+
+
+# ---- P16: Cash-Karp (RKCK, Eq. A12-A13) -------------------------------------------------------
+CK_A = [[], [Fraction(1, 5)], [Fraction(3, 40), Fraction(9, 40)], [Fraction(3, 10), Fraction(-9, 10), Fraction(6, 5)],
+        [Fraction(-11, 54), Fraction(5, 2), Fraction(-70, 27), Fraction(35, 27)],
+        [Fraction(1631, 55296), Fraction(175, 512), Fraction(575, 13824), Fraction(44275, 110592), Fraction(253, 4096)]]
+CK_B = [Fraction(37, 378), 0, Fraction(250, 621), Fraction(125, 594), 0, Fraction(512, 1771)]
+
+
+def test_P16_rkck_modified_tableau_matches_paper():
+    """Eq. A4-A7 applied to the Cash-Karp tableau reproduce the paper's a*, b* (Eq. A12-A13) entry by entry; the
+    two entries the extracted text garbles differ from the printed ones in one digit each and every row of a*
+    sums to 1 (consistency: y^(i+1) = y0 when all k vanish)."""
+    gold = json.load(open(os.path.join(GOLD, "paper_values.json")))
+    astar, bstar = modified_tableau(CK_A, CK_B)
+    assert bstar == [Fraction(s) for s in gold["rkck_b_star"]["value"]]
+    for i, row in enumerate(gold["rkck_a_star"]["value"]):
+        assert astar[i] == [Fraction(v) for v in row]
+        assert sum(astar[i]) == 1
+    assert sum(bstar) == 1
+    g = gold["rkck_a_star"]["printed_garbled"]
+    assert Fraction(g["row5_col1"]) != astar[4][0] and Fraction(g["row5_col3"]) != astar[4][2]
+    # the oracle's float tableau is that tableau
+    for i in range(6):
+        assert [float(x) for x in CK_A[i]] == list(O.RKCK_A[i])
+        assert float(CK_B[i]) == O.RKCK_B[i]
+        assert float(sum(CK_A[i], Fraction(0))) == pytest.approx(O.RKCK_C[i], abs=1e-16)
+
+
+def test_P16_rkck_is_fifth_order_and_stage_form_matches():
+    w = I.small_shell(20, 7)
+    box = O.Box(w.nx, w.ny, w.nz, w.h)
+    pot = O.Potential(w.kind, w.ax, w.ay, w.az, 5.0, 20.0, 0.05, w.omega)
+    act = O.active_indices(box, pot, w.v_cut, O.MASK_UNION)
+    grid = O.SparseGrid(box, act, 1)
+    y0 = I.make_psi0(w, act)
+    g = w.g
+    # linear test equation: amplification factor = degree-5 Taylor polynomial + z^6 b6 a65 a54 a43 a32 a21 (= z^6/800)
+    pot0 = O.Potential(kind=O.HARMONIC)
+    n, h = 12, 0.6
+    boxf, gridf = full_box_grid(n, n, n, h)
+    e1, v1 = ho_ground_state_1d(n, h, 7)
+    psi = (v1[:, None, None] * v1[None, :, None] * v1[None, None, :]).ravel().astype(np.complex128)
+    dt = 0.2
+    z = -1j * 3 * e1 * dt
+    taylor5 = sum(z ** k / math.factorial(k) for k in range(6))
+    got = O.rkck_step(gridf, pot0, 0.0, 0.0, dt, psi, 7)
+    fac = np.vdot(psi, got) / np.vdot(psi, psi)
+    c6 = CK_B[5] * CK_A[5][4] * CK_A[4][3] * CK_A[3][2] * CK_A[2][1] * CK_A[1][0]
+    assert c6 == Fraction(1, 800)
+    assert abs(fac - taylor5 - z ** 6 * float(c6)) < 1e-13
+    # order 5 on the nonlinear, ramped problem
+    T = 0.04
+    ref = O.run_rkck(grid, pot, g, 0.0, T / 64, 64, y0, 7)
+    errs = [np.max(np.abs(O.run_rkck(grid, pot, g, 0.0, T / k, k, y0, 7) - ref)) for k in (2, 4)]
+    assert 20 < errs[0] / errs[1] < 45
+    # the stage-state form with the paper's a*, b* gives the textbook step
+    astar, bstar = modified_tableau(CK_A, CK_B)
+    t, dt = 0.003, 2e-3
+    f = lambda tt, y: -1j * O.apply_H(grid, pot, g, tt, y, 7)
+    ys = [y0]
+    for i in range(1, 6):
+        nxt = sum(float(astar[i - 1][j]) * ys[j] for j in range(i)) + dt * float(CK_A[i][i - 1]) * f(t + O.RKCK_C[i - 1] * dt, ys[i - 1])
+        ys.append(nxt)
+    ynew = sum(float(bstar[j]) * ys[j] for j in range(6)) + dt * float(CK_B[5]) * f(t + O.RKCK_C[5] * dt, ys[5])
+    want = O.rkck_step(grid, pot, g, t, dt, y0, 7)
+    assert np.max(np.abs(ynew - want)) < 1e-13 * np.max(np.abs(want))

@@ -328,6 +328,11 @@ def run_ours(args, w):
     extra["imag_step"] = {"ms": ms_imag, "point_updates_per_s": n / (ms_imag * 1e-3), "GBps": 2 * csize * n / (ms_imag * 1e-3) / 1e9}
     ms_sp = timed(lambda: sim.run_imag_split(w.dt, 10), 2) / 10
     extra["imag_split_step"] = {"ms": ms_sp, "point_updates_per_s": n / (ms_sp * 1e-3), "GBps": 6 * csize * n / (ms_sp * 1e-3) / 1e9}
+    ms_h3 = timed(lambda: sim.run_rkhe3(w.dt, 5), 2) / 5
+    extra["rkhe3_step"] = {"ms": ms_h3, "stage_updates_per_s": 3 * n / (ms_h3 * 1e-3), "GBps": 9 * csize * n / (ms_h3 * 1e-3) / 1e9}
+    ms_ck = timed(lambda: sim.run_rkck(w.dt, 5), 2) / 5
+    extra["rkck_step"] = {"ms": ms_ck, "stage_updates_per_s": 6 * n / (ms_ck * 1e-3), "GBps": 27 * csize * n / (ms_ck * 1e-3) / 1e9}
+    sim.set_psi_host(host_np)
     ms_en = timed(lambda: sim.energy(), 3)
     extra["energy"] = {"ms": ms_en, "GBps": csize * n / (ms_en * 1e-3) / 1e9}
     ms_nm = timed(lambda: sim.norm(), 3)

@@ -183,6 +183,16 @@ int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 int gpe_step_rkhe3(gpe_sim* s, double dt, void* stream);
 int gpe_run_rkhe3(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 
+/* The Cash-Karp method "RKCK", fifth-order solution, in the stage-state form of Eq. A6-A7 with the
+ * modified tableau of PAPER.md:321-329 Eq. A12-A13 (two entries of the last row of a* are garbled in the
+ * extracted text; 253/12288 and 1375/1536 follow from Eq. A4-A7 and are used): six fused stage kernels per
+ * step, stage i reading the stencil operand y^(i) and, at the point itself, the earlier stage states
+ * y^(1..i-1).  Needs six stage states: the four of the caller's state block plus two that the library
+ * allocates on first use (n_active complex values each, freed by gpe_sim_destroy; OUT_OF_MEMORY if that
+ * fails).  No step-size control (the embedded fourth-order solution is not formed).  Clock as gpe_run_rk4. */
+int gpe_step_rkck(gpe_sim* s, double dt, void* stream);
+int gpe_run_rkck(gpe_sim* s, double dt, int64_t nsteps, void* stream);
+
 /* a5: psi' = psi - dt H[psi] psi, psi <- psi' sqrt(n_target / (h^3 sum|psi'|^2)) with V frozen at the sim
  * clock (PAPER.md:35, :60 Eq. 6, :87; forward-Euler reading DESIGN.md R7).  One fused kernel per step
  * (update + block partial sums) + a one-block finalise; the scale is applied lazily at the next load as

@@ -63,7 +63,7 @@ SYMBOLS = (
     "gpe_set_time", "gpe_get_time", "gpe_apply_H", "gpe_step_rk4", "gpe_run_rk4", "gpe_imag_step",
     "gpe_run_imag", "gpe_norm", "gpe_energy", "gpe_sim_kernel_launches", "gpe_sim_time_stages",
     "gpe_sim_stage_time_ms", "gpe_sim_set_planes_per_block", "gpe_imag_split_step", "gpe_run_imag_split",
-    "gpe_remap_psi", "gpe_step_rkhe3", "gpe_run_rkhe3",
+    "gpe_remap_psi", "gpe_step_rkhe3", "gpe_run_rkhe3", "gpe_step_rkck", "gpe_run_rkck",
 )
 
 _lib = None
@@ -270,6 +270,12 @@ class Sim:
 
     def run_rkhe3(self, dt, nsteps, stream=None):
         _check(lib().gpe_run_rkhe3(self._h, C.c_double(dt), C.c_int64(nsteps), _stream_ptr(stream)))
+
+    def step_rkck(self, dt, stream=None):
+        _check(lib().gpe_step_rkck(self._h, C.c_double(dt), _stream_ptr(stream)))
+
+    def run_rkck(self, dt, nsteps, stream=None):
+        _check(lib().gpe_run_rkck(self._h, C.c_double(dt), C.c_int64(nsteps), _stream_ptr(stream)))
 
     def imag_step(self, dt, stream=None):
         _check(lib().gpe_imag_step(self._h, C.c_double(dt), _stream_ptr(stream)))

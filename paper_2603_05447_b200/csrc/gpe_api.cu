@@ -34,6 +34,7 @@ struct gpe_sim {
     int64_t n = 0;          // n_active
     void* buf[4] = {nullptr, nullptr, nullptr, nullptr};  // A (psi), B, C, D in storage order
     void* staging = nullptr;                               // canonical staging (host copies, apply_H)
+    void* extra[2] = {nullptr, nullptr};                   // library-owned: two more stage states for RKCK (lazy)
     // library-owned scratch
     WorkRec* d_work = nullptr;
     int32_t n_blocks = 0;
@@ -237,6 +238,40 @@ int rkhe3_step(gpe_sim* s, double t, double dt, void* stream) {
     return GPE_OK;
 }
 
+// general stage of Eq. A6-A7: out = sum_j coef[j] aux[j] + coefc in + ca f(t, in)
+int stage_lc(gpe_sim* s, double t, double ca, const void* in, int n_aux, const void* const* aux, const double* coef,
+             double coefc, void* out, void* stream) {
+    StageParams p = base_params(s, t);
+    p.ca = ca; p.in = in; p.out1 = out;
+    p.n_aux = n_aux;
+    p.coefc = coefc;
+    for (int j = 0; j < n_aux; ++j) { p.auxn[j] = aux[j]; p.coef[j] = coef[j]; }
+    KL(launch_stage(s->dtype, s->radius, MODE_LC, p, stream));
+    if (s->n_blocks > 0) s->launches += 1;
+    return GPE_OK;
+}
+
+int rkck_step(gpe_sim* s, double t, double dt, void* stream) {
+    // Cash-Karp in the stage-state form: a*, b* of PAPER.md:321-329 Eq. A12-A13 (two garbled entries of the
+    // last row of a* corrected: 253/12288, 1375/1536; R17), a_{i+1,i} and c_i of the Cash-Karp tableau
+    void* Y[6] = {s->buf[0], s->buf[1], s->buf[2], s->buf[3], s->extra[0], s->extra[1]};
+    static const double c[6] = {0.0, 1.0 / 5.0, 3.0 / 10.0, 3.0 / 5.0, 1.0, 7.0 / 8.0};
+    static const double sub[6] = {1.0 / 5.0, 9.0 / 40.0, 6.0 / 5.0, 35.0 / 27.0, 253.0 / 4096.0, 512.0 / 1771.0};
+    static const double astar[5][5] = {
+        {1.0, 0, 0, 0, 0},
+        {5.0 / 8.0, 3.0 / 8.0, 0, 0, 0},
+        {2.0, 3.0, -4.0, 0, 0},
+        {-49.0 / 81.0, 35.0 / 27.0, 200.0 / 81.0, -175.0 / 81.0, 0},
+        {253.0 / 12288.0, -3795.0 / 4096.0, 1375.0 / 1536.0, 2875.0 / 4096.0, 1265.0 / 4096.0}};
+    static const double bstar[6] = {-991.0 / 15939.0, -3865.0 / 5313.0, 5000.0 / 5313.0, 3125.0 / 4554.0, 25.0 / 154.0, 0.0};
+    int rc;
+    for (int i = 0; i < 5; ++i) {   // y^(i+2) = sum_{j<=i} a*_{i,j} y^(j+1) + dt a_{i+2,i+1} f(t + c_{i+1} dt, y^(i+1))
+        if ((rc = stage_lc(s, t + c[i] * dt, sub[i] * dt, Y[i], i, Y, astar[i], astar[i][i], Y[i + 1], stream))) return rc;
+    }
+    // y_new = sum_{j<=5} b*_j y^(j) + dt b_6 f(t + c_6 dt, y^(6)); written over y^(1) (read at the point itself only)
+    return stage_lc(s, t + c[5] * dt, sub[5] * dt, Y[5], 5, Y, bstar, bstar[5], Y[0], stream);
+}
+
 int sums_to_host(gpe_sim* s, double out[NACC], void* stream) {
     CU(cudaMemcpyAsync(out, s->d_sums, NACC * sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CU(cudaStreamSynchronize((cudaStream_t)stream));
@@ -400,6 +435,8 @@ int gpe_sim_destroy(gpe_sim* s) {
     if (s->d_work) cudaFree(s->d_work);
     if (s->d_partials) cudaFree(s->d_partials);
     if (s->d_sums) cudaFree(s->d_sums);
+    for (int k = 0; k < 2; ++k)
+        if (s->extra[k]) cudaFree(s->extra[k]);
     for (int k = 0; k < 4; ++k)
         for (cudaEvent_t e : s->ev[k]) cudaEventDestroy(e);
     if (s->counted && s->grid && s->grid->n_sims > 0) s->grid->n_sims -= 1;
@@ -534,6 +571,29 @@ int gpe_run_rkhe3(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
 }
 
 int gpe_step_rkhe3(gpe_sim* s, double dt, void* stream) { return gpe_run_rkhe3(s, dt, 1, stream); }
+
+int gpe_run_rkck(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
+    if (s->n > 0 && nsteps > 0) {
+        for (int k = 0; k < 2; ++k) {
+            if (s->extra[k]) continue;
+            cudaError_t e = cudaMalloc(&s->extra[k], buf_bytes(s->n, s->dtype));
+            if (e == cudaErrorMemoryAllocation) return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(RKCK stage states)");
+            CU(e);
+            CU(cudaMemsetAsync(s->extra[k], 0, buf_bytes(s->n, s->dtype), (cudaStream_t)stream));
+        }
+    }
+    const double t0 = s->t;
+    for (int64_t n = 0; n < nsteps; ++n) {
+        int rc = rkck_step(s, t0 + (double)n * dt, dt, stream);
+        if (rc) return rc;
+    }
+    s->t = t0 + (double)nsteps * dt;
+    return GPE_OK;
+}
+
+int gpe_step_rkck(gpe_sim* s, double dt, void* stream) { return gpe_run_rkck(s, dt, 1, stream); }
 
 int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");

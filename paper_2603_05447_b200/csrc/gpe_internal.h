@@ -93,8 +93,11 @@ enum Mode : int {
     // the paper's own imaginary-time iteration, ca = dt/2:
     MODE_PREP = 7,   // pointwise: psi = scale * c; out1 = psi exp(-V ca) (1 - g ca |psi|^2)       (Eq. 7, lazy scale)
     MODE_KIN = 8,    // out1 = c - ca T c                                                          (first Euler half step)
-    MODE_SPLITB = 9  // u = c - ca T c; out1 = u exp(-V ca) (1 - g ca |u|^2); partial sum of |out1|^2
+    MODE_SPLITB = 9, // u = c - ca T c; out1 = u exp(-V ca) (1 - g ca |u|^2); partial sum of |out1|^2
+    // general stage of the memory-optimised Runge-Kutta form (PAPER.md:276-281 Eq. A6-A7; used for RKCK, A12-A13):
+    MODE_LC = 10     // out1 = sum_{j < n_aux} coef[j] auxn[j] + coefc c + ca * f(c)
 };
+constexpr int MAX_LC_AUX = 5;
 constexpr int NACC = 4;           // accumulators per block in the partial-sum array
 constexpr int STAGE_THREADS = 32;
 
@@ -114,6 +117,11 @@ struct StageParams {
     double hax, hay, haz;  // 0.5 a_x, 0.5 a_y, 0.5 a_z
     double om2;            // Omega^2
     double delta_eff;      // Delta(t) for the dressed potential, 0 for the harmonic one
+    const void* auxn[5];   // MODE_LC: earlier stage states y^(j) (storage order), read at the point itself only
+    double coef[5];        // MODE_LC: a*_{ij} (or b*_j) of those states
+    double coefc;          // MODE_LC: a*_{ii} (or b*_i) of the stage state c the stencil is applied to
+    int32_t n_aux;         // MODE_LC: number of entries of auxn / coef in use
+    int32_t pad_lc;
     double comb[3];        // MODE_S2: out2 = comb[0] aux + comb[1] c + comb[2] out1 (the b* terms known so far, Eq. A7)
     const void* in;        // array the stencil is applied to (storage order)
     const void* aux;       // y0 or p (storage order) or null

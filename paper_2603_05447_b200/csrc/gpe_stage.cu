@@ -137,7 +137,7 @@ template <> struct KW<float> {
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
 
 template <typename T, int R, int MODE, int PR>
-__global__ void __launch_bounds__(STAGE_THREADS, (PR == 2 ? 16 : (sizeof(T) == 8 ? 12 : 16)))
+__global__ void __launch_bounds__(STAGE_THREADS, 16)
 stage_kernel(const __grid_constant__ StageParams p) {
     using C = typename CxOf<T>::type;
     constexpr bool HAS_AUX = mode_has_aux(MODE);
@@ -326,6 +326,29 @@ stage_kernel(const __grid_constant__ StageParams p) {
             cbase = lds_u1(sbase + (unsigned)ic * 4u) + (ghi ? (unsigned)__popc(m.x) : 0u);
             cany = (m.x | m.y) != 0u;
         }
+        // ---- MODE_LC: the earlier stage states of plane c, plain loads issued before anything else of the step ----
+        C lcs[PR];
+        if (MODE == MODE_LC) {
+#pragma unroll
+            for (int e = 0; e < PR; ++e) lcs[e] = mk<T>((T)0, (T)0);
+            if (cany) {
+#pragma unroll
+                for (int j = 0; j < MAX_LC_AUX; ++j) {
+                    if (j < p.n_aux) {
+                        const C* __restrict__ aj = reinterpret_cast<const C*>(p.auxn[j]);
+                        const T cj = (T)p.coef[j];
+#pragma unroll
+                        for (int e = 0; e < PR; ++e) {
+                            if ((cword >> (rb0 + 8 * e)) & 1u) {
+                                const C a = __ldg(aj + (cbase + (unsigned)__popc(cword & bm[e])));
+                                lcs[e].x = fma(cj, a.x, lcs[e].x);
+                                lcs[e].y = fma(cj, a.y, lcs[e].y);
+                            }
+                        }
+                    }
+                }
+            }
+        }
         // ---- psi(k) of the patch ------------------------------------------------------------------------
         C v[PR];
 #pragma unroll
@@ -406,6 +429,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     o = mk<T>(s * fma(-ca, hc.x, cv.x), s * fma(-ca, hc.y, cv.y));
                     const double o2 = (double)o.x * (double)o.x + (double)o.y * (double)o.y;
                     acc[0] += on ? o2 : 0.0;
+                } else if (MODE == MODE_LC) {
+                    const T cc = (T)p.coefc;
+                    o = mk<T>(fma(ca, hc.y, fma(cc, cv.x, lcs[e].x)), fma(-ca, hc.x, fma(cc, cv.y, lcs[e].y)));
                 } else {
                     // f = -i H c = (hc.y, -hc.x)
                     const C base = (MODE == MODE_S1) ? cv : av[e];
@@ -533,6 +559,7 @@ cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
         case MODE_PREP: return launch_one<T, R, MODE_PREP>(p, st);
         case MODE_KIN: return launch_one<T, R, MODE_KIN>(p, st);
         case MODE_SPLITB: return launch_one<T, R, MODE_SPLITB>(p, st);
+        case MODE_LC: return launch_one<T, R, MODE_LC>(p, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -555,6 +582,7 @@ cudaError_t set_attr_modes() {
     if ((e = set_attr<T, R, MODE_PREP>())) return e;
     if ((e = set_attr<T, R, MODE_KIN>())) return e;
     if ((e = set_attr<T, R, MODE_SPLITB>())) return e;
+    if ((e = set_attr<T, R, MODE_LC>())) return e;
     return cudaSuccess;
 }
 

@@ -232,3 +232,24 @@ def test_rkhe3_small_shell_with_ramp(P, stencil, dtype):
     assert abs(sim.time - (0.005 + 5 * w.dt)) < 1e-15
     ref = O.run_rkhe3(og, pot, w.g, 0.005, w.dt, 5, psi.astype(np.complex128), stencil)
     assert rel_max(sim.get_psi_host(), ref) < (1e-12 if dtype == "complex128" else 1e-5)
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_rkck_small_shell_with_ramp(P, stencil, dtype):
+    """Cash-Karp in the paper's stage-state form (PAPER.md Eq. A6-A7, A12-A13) against the textbook k1..k6
+    oracle, time-ramped potential (stage times t + c_i dt)."""
+    w = I.small_shell(40, stencil, dtype).with_(delta0=14.0, delta1=22.0, t_ramp=0.02)
+    box, pot, act, grid, sim = _make(P, w)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    sim.time = 0.005
+    sim.run_rkck(w.dt, 2)
+    sim.step_rkck(w.dt)
+    ref = O.run_rkck(og, pot, w.g, 0.005, w.dt, 3, psi.astype(np.complex128), stencil)
+    assert rel_max(sim.get_psi_host(), ref) < (1e-12 if dtype == "complex128" else 2e-5)
+    # the other integrators still run on the same sim afterwards (buffers A-D are shared)
+    sim.run_rk4(w.dt, 1)
+    ref = O.run_rk4(og, pot, w.g, 0.005 + 3 * w.dt, w.dt, 1, ref, stencil)
+    assert rel_max(sim.get_psi_host(), ref) < (1e-12 if dtype == "complex128" else 2e-5)

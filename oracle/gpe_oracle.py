@@ -189,11 +189,57 @@ class SparseGrid:
                 self.nbr[(axis, s)] = np.where(hit, pos_c, -1).astype(np.int64)
 
 
+def neighbour_lookup(grid: SparseGrid, off) -> np.ndarray:
+    """Position in ``active`` of the point at offset off = (dx, dy, dz) from every active point, -1 if that
+    point is outside the box or outside M."""
+    box = grid.box
+    ix, iy, iz = unravel(box, grid.active)
+    cx, cy, cz = ix + off[0], iy + off[1], iz + off[2]
+    inside = (cx >= 0) & (cx < box.nx) & (cy >= 0) & (cy < box.ny) & (cz >= 0) & (cz < box.nz)
+    target = (cx * box.ny + cy) * box.nz + cz
+    pos = np.searchsorted(grid.active, target)
+    pos_c = np.minimum(pos, max(grid.n - 1, 0))
+    hit = inside & (pos < grid.n)
+    if grid.n:
+        hit &= grid.active[pos_c] == target
+    return np.where(hit, pos_c, -1)
+
+
+def apply_T19(grid: SparseGrid, psi: np.ndarray) -> np.ndarray:
+    """T psi = -1/2 lap_19 psi with the 19-point higher-order compact Laplacian of PAPER.md:341-343 Eq. B2 for
+    dx = dy = dz = h:  lap_19 = lap_7 + (h^2/6) (dxx dyy + dxx dzz + dyy dzz),  d_ii = [1,-2,1]/h^2, written out
+    term by term as in Eq. B2 (products of second differences), psi = 0 outside M."""
+    psi = np.asarray(psi, dtype=np.complex128)
+    h2 = grid.box.h * grid.box.h
+    ext = np.concatenate([psi, np.zeros(1, np.complex128)])   # index -1 -> 0
+    d2 = (1.0, -2.0, 1.0)
+
+    def term(wx, wy, wz):
+        """sum over offsets of wx[dx] wy[dy] wz[dz] psi(p + (dx,dy,dz)); w = None is the identity [0,1,0]."""
+        out = np.zeros_like(psi)
+        for dx in (-1, 0, 1):
+            for dy in (-1, 0, 1):
+                for dz in (-1, 0, 1):
+                    c = 1.0
+                    for wgt, d in ((wx, dx), (wy, dy), (wz, dz)):
+                        c *= (d2[d + 1] / h2) if wgt else (1.0 if d == 0 else 0.0)
+                    if c != 0.0:
+                        out = out + c * ext[neighbour_lookup(grid, (dx, dy, dz))]
+        return out
+
+    lap7 = term(True, False, False) + term(False, True, False) + term(False, False, True)
+    cross = term(True, True, False) + term(True, False, True) + term(False, True, True)
+    return -0.5 * (lap7 + (1.0 / 12.0) * (2.0 * h2) * cross)
+
+
 def apply_T(grid: SparseGrid, psi: np.ndarray, stencil: int) -> np.ndarray:
     """T psi = -1/2 lap_h psi on M with psi = 0 outside M (weights R5).
 
     (lap_h psi)_p = (1/h^2) sum_axis sum_{s=-R..R} c_|s| psi(p + s e_axis).
+    stencil = 19: the paper's higher-order compact Laplacian (apply_T19).
     """
+    if stencil == 19:
+        return apply_T19(grid, psi)
     w = STENCIL_WEIGHTS[stencil]
     R = len(w) - 1
     assert R <= grid.radius

@@ -21,4 +21,4 @@ def rel_max(a, b):
     return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
 
 
-RADIUS = {7: 1, 13: 2}
+RADIUS = {7: 1, 13: 2, 19: 1}

@@ -652,3 +652,52 @@ def test_P16_rkck_is_fifth_order_and_stage_form_matches():
     ynew = sum(float(bstar[j]) * ys[j] for j in range(6)) + dt * float(CK_B[5]) * f(t + O.RKCK_C[5] * dt, ys[5])
     want = O.rkck_step(grid, pot, g, t, dt, y0, 7)
     assert np.max(np.abs(ynew - want)) < 1e-13 * np.max(np.abs(want))
+
+
+# ---- P17: the 19-point higher-order compact stencil (PAPER.md:341-343 Eq. B2) ----------------------------------
+def test_P17_19pt_weights_symbol_and_kronecker():
+    gold = json.load(open(os.path.join(GOLD, "paper_values.json")))["nineteen_point_isotropic"]["value"]
+    n, h = 7, 0.5
+    box, grid = full_box_grid(n, n, n, h, radius=1)
+    # (a) weights: apply to a unit vector at the centre of the box
+    c = (n // 2 * n + n // 2) * n + n // 2
+    e = np.zeros(n ** 3, np.complex128)
+    e[c] = 1.0
+    lap = (-2.0 * O.apply_T(grid, e, 19)).real.reshape(n, n, n) * h * h
+    m = n // 2
+    assert abs(lap[m, m, m] - float(Fraction(gold["centre"]))) < 1e-13
+    for off in [(1, 0, 0), (0, -1, 0), (0, 0, 1)]:
+        assert abs(lap[m + off[0], m + off[1], m + off[2]] - float(Fraction(gold["face"]))) < 1e-13
+    for off in [(1, 1, 0), (-1, 0, 1), (0, 1, -1)]:
+        assert abs(lap[m + off[0], m + off[1], m + off[2]] - float(Fraction(gold["edge"]))) < 1e-13
+    assert abs(lap[m + 1, m + 1, m + 1]) == 0 and np.count_nonzero(lap) == 19 and abs(lap.sum()) < 1e-12
+    # (b) sine modes of the Dirichlet box are exact eigenvectors: s_x + s_y + s_z + h^2/6 (s_x s_y + s_x s_z + s_y s_z)
+    mode = (2, 1, 3)
+    psi = sine_mode(n, n, n, mode).ravel()
+    sx, sy, sz = [-(4 / h ** 2) * math.sin(math.pi * mm / (2 * (n + 1))) ** 2 for mm in mode]
+    lam = sx + sy + sz + h * h / 6 * (sx * sy + sx * sz + sy * sz)
+    assert np.max(np.abs(O.apply_T(grid, psi, 19) + 0.5 * lam * psi)) < 1e-12
+    # (c) Eq. B2 as Kronecker products with rows / columns deleted, random masks
+    nx, ny, nz = 5, 6, 4
+    d = lambda k: lap1d(k, h, 7)
+    eye = np.eye
+    k3 = lambda a, b, cc: np.kron(np.kron(a, b), cc)
+    lap7 = k3(d(nx), eye(ny), eye(nz)) + k3(eye(nx), d(ny), eye(nz)) + k3(eye(nx), eye(ny), d(nz))
+    lap19 = lap7 + (2 * h * h / 12) * (k3(d(nx), d(ny), eye(nz)) + k3(d(nx), eye(ny), d(nz)) + k3(eye(nx), d(ny), d(nz)))
+    for seed, pr in ((31, 0.6), (32, 0.9)):
+        act = I.random_mask_lin(seed, nx, ny, nz, pr)
+        tmat = -0.5 * lap19[np.ix_(act, act)]
+        g2 = O.SparseGrid(O.Box(nx, ny, nz, h), act, 1)
+        psi = I.random_psi(seed, act.size)
+        assert np.max(np.abs(O.apply_T(g2, psi, 19) - tmat @ psi)) < 1e-12 * np.max(np.abs(tmat)) * 8
+        assert np.max(np.abs(tmat - tmat.T)) == 0          # Hermitian (principal sub-matrix)
+
+
+def test_P17_19pt_leading_error_is_isotropic():
+    """lap_19 u = lap u + h^2/12 lap^2 u + O(h^4): on a plane wave the symbol is -k^2 + h^2 k^4 / 12 to that order,
+    a function of |k| only (the 7-point symbol has h^2/12 sum k_i^4 instead)."""
+    h = 0.05
+    for kv in ((1.0, 2.0, 2.0), (3.0, 0.0, 0.0), (0.0, 2.4, 1.8)):      # all |k| = 3
+        s = [-(4 / h ** 2) * math.sin(k * h / 2) ** 2 for k in kv]
+        lam19 = sum(s) + h * h / 6 * (s[0] * s[1] + s[0] * s[2] + s[1] * s[2])
+        assert abs(lam19 - (-9.0 + h * h * 81.0 / 12)) < 5e-5 * 9

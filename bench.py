@@ -39,6 +39,8 @@ def workloads():
     return {
         "cfg4_c128": I.config4("complex128"),
         "cfg4_c64": I.config4("complex64"),
+        "cfg4_19pt_c128": I.config4("complex128").with_(stencil=19, name="cfg4_ellipsoid_1024_19pt_c128"),
+        "cfg3b_19pt": I.config3(False).with_(stencil=19, name="cfg3b_ramp_final_512_19pt"),
         "cfg2": I.config2().with_(dt=1e-4),
         "cfg3a": I.config3(True),
         "cfg3b": I.config3(False),

@@ -145,7 +145,9 @@ int gpe_grid_layout_tables(const gpe_grid* g, const gpe_layout_tables* out_host)
  * p of PAPER.md:276-281 Eq. A6-A7 specialised to RK4), one canonical staging buffer, reduction scratch. */
 int gpe_sim_state_bytes(const gpe_grid* g, int dtype, size_t* out);
 
-/* stencil: 7 (2nd order, PAPER.md:58, :337-339 Eq. B1) or 13 (4th-order star, R5).
+/* stencil: 7 (2nd order, PAPER.md:58, :337-339 Eq. B1), 13 (4th-order star, R5) or 19 (the paper's
+ * higher-order compact Laplacian for dx = dy = dz = h, PAPER.md:341-343 Eq. B2: centre -4/h^2, faces 1/3h^2,
+ * edges 1/6h^2; radius 1 plus the twelve edge neighbours, zero outside M like every other read).
  * g: interaction strength multiplying |psi|^2; n_target: value of h^3 sum|psi|^2 that imaginary-time
  * steps renormalise to (Eq. 3).  dev_state: device memory, 256-byte aligned, >= state_bytes,
  * must stay valid until gpe_sim_destroy; it is zero-initialised here (psi = 0, t = 0).  Uploads the

@@ -27,6 +27,7 @@ struct gpe_sim {
     gpe_grid* grid = nullptr;
     int dtype = GPE_C128;
     int radius = 1;
+    bool hoc = false;       // 19-point higher-order compact stencil (radius 1 plus edge neighbours)
     double g = 0.0, n_target = 1.0;
     double t = 0.0;
     int kz = 32;
@@ -107,8 +108,21 @@ int build_work(gpe_sim* s) {
             r.eoff[0] = h.tile_entry_base[k] - h.tile_zlo[k];
             r.zlo[0] = h.tile_zlo[k];
             r.zhi[0] = h.tile_zhi[k];
-            for (int q = 1; q <= 4; ++q) {
-                const int32_t nb = h.tile_nbr[4 * k + q - 1];
+            for (int q = 1; q < NTILE; ++q) {
+                int32_t nb = -1;
+                if (q <= 4) {
+                    nb = h.tile_nbr[4 * k + q - 1];
+                } else {
+                    // diagonal tile (i +- 1, j +- 1): the tile list ascends in (i, j), binary search
+                    const int32_t ti = h.tile_xy[2 * k] + (q <= 6 ? -1 : 1), tj = h.tile_xy[2 * k + 1] + ((q & 1) ? -1 : 1);
+                    int64_t lo = 0, hi = h.n_tiles();
+                    while (lo < hi) {
+                        const int64_t mid = (lo + hi) / 2;
+                        const int32_t mi = h.tile_xy[2 * mid], mj = h.tile_xy[2 * mid + 1];
+                        if (mi < ti || (mi == ti && mj < tj)) lo = mid + 1; else hi = mid;
+                    }
+                    if (lo < h.n_tiles() && h.tile_xy[2 * lo] == ti && h.tile_xy[2 * lo + 1] == tj) nb = (int32_t)lo;
+                }
                 if (nb >= 0) {
                     r.eoff[q] = h.tile_entry_base[nb] - h.tile_zlo[nb];
                     r.zlo[q] = h.tile_zlo[nb];
@@ -179,6 +193,11 @@ StageParams base_params(const gpe_sim* s, double t) {
     p.kw[0] = ih2 * 3.0 * (s->radius == 1 ? -2.0 : -2.5);
     p.kw[1] = ih2 * (s->radius == 1 ? 1.0 : 4.0 / 3.0);
     p.kw[2] = s->radius == 1 ? 0.0 : ih2 * (-1.0 / 12.0);
+    if (s->hoc) {   // PAPER.md:343 Eq. B2 with dx = dy = dz = h: centre -4, faces 1/3, edges 1/6 (over h^2)
+        p.kw[0] = ih2 * -4.0;
+        p.kw[1] = ih2 * (1.0 / 3.0);
+        p.kw[2] = ih2 * (1.0 / 6.0);
+    }
     for (int k = 0; k < 3; ++k) p.kwf[k] = (float)p.kw[k];
     p.xc = 0.5 * (double)(h.box.nx - 1);
     p.yc = 0.5 * (double)(h.box.ny - 1);
@@ -205,11 +224,11 @@ int stage(gpe_sim* s, int mode, double t, double ca, const void* in, const void*
             v.push_back(e);
         }
         CU(cudaEventRecord(v[u], st));
-        KL(launch_stage(s->dtype, s->radius, mode, p, stream));
+        KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, mode, p, stream));
         CU(cudaEventRecord(v[u + 1], st));
         u += 2;
     } else {
-        KL(launch_stage(s->dtype, s->radius, mode, p, stream));
+        KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, mode, p, stream));
     }
     if (s->n_blocks > 0) s->launches += 1;
     return GPE_OK;
@@ -246,7 +265,7 @@ int stage_lc(gpe_sim* s, double t, double ca, const void* in, int n_aux, const v
     p.n_aux = n_aux;
     p.coefc = coefc;
     for (int j = 0; j < n_aux; ++j) { p.auxn[j] = aux[j]; p.coef[j] = coef[j]; }
-    KL(launch_stage(s->dtype, s->radius, MODE_LC, p, stream));
+    KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, MODE_LC, p, stream));
     if (s->n_blocks > 0) s->launches += 1;
     return GPE_OK;
 }
@@ -389,9 +408,9 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
                    size_t state_bytes, void* stream, gpe_sim** out) {
     if (!g || !dev_state || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
     if (dtype != GPE_C64 && dtype != GPE_C128) return fail(GPE_ERR_INVALID_ARG, "unknown dtype");
-    if (stencil != 7 && stencil != 13) return fail(GPE_ERR_INVALID_ARG, "stencil must be 7 or 13");
+    if (stencil != 7 && stencil != 13 && stencil != 19) return fail(GPE_ERR_INVALID_ARG, "stencil must be 7, 13 or 19");
     if (!(n_target > 0.0)) return fail(GPE_ERR_INVALID_ARG, "n_target must be > 0");
-    const int radius = stencil == 7 ? 1 : 2;
+    const int radius = stencil == 13 ? 2 : 1;
     if (g->h.tx != 8 || g->h.ty != 8) return fail(GPE_ERR_UNSUPPORTED, "kernels need 8x8 column tiles");
     if (g->h.halo_width < radius) return fail(GPE_ERR_UNSUPPORTED, "grid halo_width is smaller than the stencil radius");
     if (g->h.n_active >= ((int64_t)1 << 32)) return fail(GPE_ERR_UNSUPPORTED, "more than 2^32-1 active points (kernels index storage with 32 bits)");
@@ -405,6 +424,7 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     s->grid = g;
     s->dtype = dtype;
     s->radius = radius;
+    s->hoc = stencil == 19;
     s->g = g_int;
     s->n_target = n_target;
     s->csize = dtype == GPE_C128 ? 16 : 8;

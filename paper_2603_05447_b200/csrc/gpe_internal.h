@@ -59,19 +59,21 @@ struct Slab {                // one z-plane of one tile
 };
 
 // One stream (a warp's worth of work): nz consecutive planes of one tile (a piece of a work item).
-// eoff[q] + zp = slab entry of plane zp in tile q (0 = own, 1..4 = -x,+x,-y,+y), valid for
+// eoff[q] + zp = slab entry of plane zp in tile q (0 = own, 1..4 = -x,+x,-y,+y, 5..8 = the diagonal tiles
+// (-x,-y), (-x,+y), (+x,-y), (+x,+y) whose corner points the 19-point stencil reads), valid for
 // zlo[q] <= zp < zhi[q] (zlo = zhi = 0 when the neighbour tile is absent).
+constexpr int NTILE = 9;
 struct alignas(16) WorkRec {
     int32_t ix0, iy0;   // box index of the tile's (lx,ly) = (0,0) column
     int32_t z0, nz;
-    long long eoff[5];
-    int32_t zlo[5];
-    int32_t zhi[5];
+    long long eoff[NTILE];
+    int32_t zlo[NTILE];
+    int32_t zhi[NTILE];
     long long pos0;     // storage position of the first point of the piece
     int32_t npts;       // points in the piece (contiguous in storage from pos0)
-    int32_t pad[5];
+    int32_t pad[3];
 };
-static_assert(sizeof(WorkRec) == 128, "WorkRec layout");
+static_assert(sizeof(WorkRec) == 192, "WorkRec layout");
 
 struct PotDev {
     int32_t kind;
@@ -110,7 +112,7 @@ struct StageParams {
     double g;
     double ca;             // stage coefficient (dt/2, dt, dt/6, or dt of the imaginary step)
     // host-precomputed constants (read from the parameter bank, no registers):
-    double kw[3];          // -1/(2h^2) * {3 c_0, c_1, c_2} of the stencil
+    double kw[3];          // -1/(2h^2) * {3 c_0, c_1, c_2} of the star stencils; 19-point: * {centre, face, edge} weights
     float kwf[3];          // the same in fp32 (complex64 state)
     float padf;
     double xc, yc, zc;     // 0.5 (n-1) per axis: coordinate = (i - xc) h + cx
@@ -132,8 +134,9 @@ struct StageParams {
 };
 
 // Launchers (gpe_kernels.cu).  dtype: GPE_C64 / GPE_C128; radius 1 or 2.  Return cudaError_t as int.
-int launch_stage(int dtype, int radius, int mode, const StageParams& p, void* stream);
-size_t stage_smem_bytes(int dtype, int radius);
+// variant: 1 = 7-point, 2 = 13-point, 3 = 19-point higher-order compact (radius 1 + in-plane / z diagonals)
+int launch_stage(int dtype, int variant, int mode, const StageParams& p, void* stream);
+size_t stage_smem_bytes(int dtype, int variant);
 int stage_max_planes();   // upper bound of WorkRec::nz the stage kernels accept
 int launch_pack(int dtype, const void* canonical, void* storage, const int64_t* perm, int64_t n, void* stream);
 int launch_unpack(int dtype, const void* storage, void* canonical, const int64_t* perm, int64_t n, void* stream);

@@ -109,7 +109,8 @@ constexpr int STAGE_WARPS = STAGE_THREADS / 32;
 
 // Shared memory of one stream.  Plane slot: (8+2R) rows (x) of PY values, the tile at rows/cols R..R+7 and
 // the star halo around it.
-template <typename T, int R, bool AUX> struct Geo {
+template <typename T, int R, bool AUX, bool HOC = false> struct Geo {
+    static constexpr int NT = HOC ? NTILE : 5;               // tiles whose slab tables are staged
     static constexpr int ES = 2 * (int)sizeof(T);
     static constexpr int ROWS = 8 + 2 * R;
     // row pitch in values; 8-byte values are read by half-warps (two rows, 2 apart): 2 PY 8 = 64 (mod 128) bytes
@@ -120,9 +121,9 @@ template <typename T, int R, bool AUX> struct Geo {
     static constexpr int NAUX = pf_of(R) + 1;               // ring of aux-plane slots per stream
     static constexpr int RING_BYTES = NSLOT * PLANE * ES;
     static constexpr int AUX_BYTES = AUX ? NAUX * 64 * ES : 0;
-    static constexpr int MASK_OFF = RING_BYTES + AUX_BYTES;  // [5][NE] (lo, hi)
-    static constexpr int BASE_OFF = MASK_OFF + 5 * NE * 8;   // [5][NE] storage base
-    static constexpr int STREAM_BYTES = (BASE_OFF + 5 * NE * 4 + 15) / 16 * 16;
+    static constexpr int MASK_OFF = RING_BYTES + AUX_BYTES;  // [NT][NE] (lo, hi)
+    static constexpr int BASE_OFF = MASK_OFF + NT * NE * 8;  // [NT][NE] storage base
+    static constexpr int STREAM_BYTES = (BASE_OFF + NT * NE * 4 + 15) / 16 * 16;
     __host__ __device__ static constexpr int at(int r, int c) { return (r + R) * PY + (c + R); }
 };
 
@@ -136,12 +137,14 @@ template <> struct KW<float> {
 
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
 
-template <typename T, int R, int MODE, int PR>
+template <typename T, int R, int MODE, int PR, bool HOC>
 __global__ void __launch_bounds__(STAGE_THREADS, 16)
 stage_kernel(const __grid_constant__ StageParams p) {
+    static_assert(!HOC || (R == 1 && PR == 2), "the 19-point stencil has radius 1 and runs with a warp per stream");
     using C = typename CxOf<T>::type;
     constexpr bool HAS_AUX = mode_has_aux(MODE);
-    using G = Geo<T, R, HAS_AUX>;
+    using G = Geo<T, R, HAS_AUX, HOC>;
+    constexpr int NT = G::NT;
     constexpr int PF = pf_of(R), NSLOT = G::NSLOT, NAUX = G::NAUX;
     constexpr unsigned ES = G::ES;
     constexpr int LPS = 64 / PR;                           // lanes per stream (16: half-warp, 32: warp)
@@ -169,9 +172,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
     // ---- slab tables of the five tiles -> shared memory (all loads in flight at once) ----------------
     {
         constexpr int NM = (G::NE + LPS - 1) / LPS;
-        unsigned tl[5 * NM], th[5 * NM], tb[5 * NM];
+        unsigned tl[NT * NM], th[NT * NM], tb[NT * NM];
 #pragma unroll
-        for (int q = 0; q < 5; ++q) {
+        for (int q = 0; q < NT; ++q) {
             const int zl = w->zlo[q], zh = w->zhi[q];
             const Slab* __restrict__ tab = p.slabs + w->eoff[q];
 #pragma unroll
@@ -185,7 +188,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
             }
         }
 #pragma unroll
-        for (int q = 0; q < 5; ++q)
+        for (int q = 0; q < NT; ++q)
 #pragma unroll
             for (int m = 0; m < NM; ++m) {
                 const int i = t + LPS * m;
@@ -226,6 +229,10 @@ stage_kernel(const __grid_constant__ StageParams p) {
         hoff[e] = (unsigned)((drow + R) * G::PY + (dcol + R)) * ES;
     }
 
+    // 19-point: lanes 0..3 fetch the corner (-x,-y), (-x,+y), (+x,-y), (+x,+y): local point (7,7), (7,0), (0,7), (0,0)
+    // of the diagonal tile, bit cbit of its high (t < 2) or low mask word
+    const int cbit = t == 0 ? 31 : (t == 1 ? 24 : (t == 2 ? 7 : 0));
+    const unsigned coff = (unsigned)G::at((t & 2) ? 8 : -1, (t & 1) ? 8 : -1) * ES;
     const C* __restrict__ in = reinterpret_cast<const C*>(p.in);
     const C* __restrict__ auxp = reinterpret_cast<const C*>(p.aux);
 
@@ -261,7 +268,8 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     cp_async_zfill(dst + (unsigned)e * ROW_BYTES, in + (bc + (unsigned)__popc(word & bm[e])), on);
                 }
             }
-            if (MODE != MODE_PREP && i >= R && i < ne - R) {
+            // 19-point: the overlap planes need their in-plane face sums too (they are the xz / yz edge neighbours)
+            if (MODE != MODE_PREP && (HOC || (i >= R && i < ne - R))) {
                 const unsigned ti = (unsigned)((1 + hq) * G::NE + i);
                 const uint2 m = lds_u2(smask + ti * 8u);
                 const unsigned b = lds_u1(sbase + ti * 4u);
@@ -273,6 +281,14 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     const bool on = (ww & (hbm[e] + 1u)) != 0u;
                     cp_async_zfill(dst + hoff[e], in + (bb + (unsigned)__popc(ww & hbm[e])), on);
                 }
+            }
+            if (HOC && MODE != MODE_PREP && t < 4) {
+                // corner of the star-plus-diagonals halo: one point of the diagonal tile 5 + t
+                const unsigned ti = (unsigned)((5 + t) * G::NE + i);
+                const uint2 m = lds_u2(smask + ti * 8u);
+                const unsigned ww = t < 2 ? m.y : m.x;
+                const unsigned pos = lds_u1(sbase + ti * 4u) + (t < 2 ? (unsigned)__popc(m.x) : 0u) + (unsigned)__popc(ww & ((1u << cbit) - 1u));
+                cp_async_zfill(ring + sp * SLOT_BYTES + coff, in + pos, (ww >> cbit) & 1u);
             }
             if (HAS_AUX) {
                 const int ia = i - R;
@@ -298,6 +314,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
 #pragma unroll
         for (int e = 0; e < PR; ++e) { SP[s][e] = mk<T>((T)0, (T)0); SA[s][e] = mk<T>((T)0, (T)0); }
     double acc[NACC] = {0.0, 0.0, 0.0, 0.0};
+    C FPV[PR];                                             // 19-point: in-plane face sum of the previous plane
+#pragma unroll
+    for (int e = 0; e < PR; ++e) FPV[e] = mk<T>((T)0, (T)0);
 
     // ---- prologue: planes 0 .. PF-1 in flight ----------------------------------------------------------------
 #pragma unroll
@@ -366,6 +385,22 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 for (int e = 0; e < PR; ++e) vpot[e] = fast_sqrt(fma(vpot[e], vpot[e], p.om2)) - p.pot.omega;
             }
         }
+        // ---- 19-point: in-plane face sum F and diagonal sum E of the patch points in plane k -------------------
+        C F[PR], E[PR];
+        if (HOC && MODE != MODE_PREP) {
+            C Lc[4], Rc[4], Mc[4];                              // columns ly-1, ly+1, ly of rows -1 .. 2 of the patch
+#pragma unroll
+            for (int r = -1; r <= 2; ++r) {
+                Lc[r + 1] = lds_c(so + (unsigned)(r * (int)ROW_BYTES - (int)ES), (C*)nullptr);
+                Rc[r + 1] = lds_c(so + (unsigned)(r * (int)ROW_BYTES + (int)ES), (C*)nullptr);
+                Mc[r + 1] = (r == 0 || r == 1) ? v[r == 1 ? 1 : 0] : lds_c(so + (unsigned)(r * (int)ROW_BYTES), (C*)nullptr);
+            }
+#pragma unroll
+            for (int a = 0; a < PR; ++a) {
+                F[a] = mk<T>((Mc[a].x + Mc[a + 2].x) + (Lc[a + 1].x + Rc[a + 1].x), (Mc[a].y + Mc[a + 2].y) + (Lc[a + 1].y + Rc[a + 1].y));
+                E[a] = mk<T>((Lc[a].x + Rc[a].x) + (Lc[a + 2].x + Rc[a + 2].x), (Lc[a].y + Rc[a].y) + (Lc[a + 2].y + Rc[a + 2].y));
+            }
+        }
         // ---- psi(k) completes the z part of planes k-1 .. k-R -------------------------------------------
 #pragma unroll
         for (int e = 0; e < PR; ++e) {
@@ -374,6 +409,10 @@ stage_kernel(const __grid_constant__ StageParams p) {
             if (R == 2) {
                 AN[e].x = fma(KW<T>::w(p, 1), v[e].x, AN[e].x);
                 AN[e].y = fma(KW<T>::w(p, 1), v[e].y, AN[e].y);
+            }
+            if (HOC && MODE != MODE_PREP) {                     // the xz / yz edge neighbours of plane k-1 in plane k
+                AO[e].x = fma(KW<T>::w(p, 2), F[e].x, AO[e].x);
+                AO[e].y = fma(KW<T>::w(p, 2), F[e].y, AO[e].y);
             }
         }
         // ---- finish plane c = k - R: nonlinear term, stage combination (branch-free; stores predicated) ----
@@ -466,9 +505,15 @@ stage_kernel(const __grid_constant__ StageParams p) {
             AO[e].x = fma(KW<T>::w(p, 0), v[e].x, an.x);
             AO[e].y = fma(KW<T>::w(p, 0), v[e].y, an.y);
             PO[e] = v[e];
+            if (HOC && MODE != MODE_PREP) {
+                // faces of plane k, and the edges: diagonals of plane k + face sum of plane k-1
+                AO[e].x = fma(KW<T>::w(p, 1), F[e].x, fma(KW<T>::w(p, 2), E[e].x + FPV[e].x, AO[e].x));
+                AO[e].y = fma(KW<T>::w(p, 1), F[e].y, fma(KW<T>::w(p, 2), E[e].y + FPV[e].y, AO[e].y));
+                FPV[e] = F[e];
+            }
         }
         // ---- in-plane part (only planes of the stream itself are ever finished) ----------------------------------
-        if (MODE != MODE_PREP && i >= R && i < ne - R) {
+        if (!HOC && MODE != MODE_PREP && i >= R && i < ne - R) {
             // x direction: source rows r = -R .. PR-1+R of column ly; rows 0..PR-1 are the patch itself
 #pragma unroll
             for (int r = -R; r <= PR - 1 + R; ++r) {
@@ -534,55 +579,55 @@ stage_kernel(const __grid_constant__ StageParams p) {
 // 9.8e10 stage updates/s on cfg 4 against 1.2e11 with 2 rows (twice the shared memory per warp: 11 warps per SM)
 template <typename T> constexpr int rows_per_lane() { return 2; }
 
-template <typename T, int R, int MODE> constexpr size_t stage_smem() {
-    return (size_t)(STAGE_WARPS * rows_per_lane<T>() / 2) * Geo<T, R, mode_has_aux(MODE)>::STREAM_BYTES;
+template <typename T, int R, int MODE, bool HOC> constexpr size_t stage_smem() {
+    return (size_t)(STAGE_WARPS * rows_per_lane<T>() / 2) * Geo<T, R, mode_has_aux(MODE), HOC>::STREAM_BYTES;
 }
 
-template <typename T, int R, int MODE>
+template <typename T, int R, int MODE, bool HOC>
 cudaError_t launch_one(const StageParams& p, cudaStream_t st) {
     constexpr int spb = STAGE_WARPS * rows_per_lane<T>() / 2;   // streams per block
     const int nblk = (p.n_work + spb - 1) / spb;
-    stage_kernel<T, R, MODE, rows_per_lane<T>()><<<nblk, STAGE_THREADS, stage_smem<T, R, MODE>(), st>>>(p);
+    stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC><<<nblk, STAGE_THREADS, stage_smem<T, R, MODE, HOC>(), st>>>(p);
     return cudaGetLastError();
 }
 
-template <typename T, int R>
+template <typename T, int R, bool HOC>
 cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
     switch (mode) {
-        case MODE_APPLY: return launch_one<T, R, MODE_APPLY>(p, st);
-        case MODE_S1: return launch_one<T, R, MODE_S1>(p, st);
-        case MODE_S2: return launch_one<T, R, MODE_S2>(p, st);
-        case MODE_S3: return launch_one<T, R, MODE_S3>(p, st);
-        case MODE_S4: return launch_one<T, R, MODE_S4>(p, st);
-        case MODE_IMAG: return launch_one<T, R, MODE_IMAG>(p, st);
-        case MODE_ENERGY: return launch_one<T, R, MODE_ENERGY>(p, st);
-        case MODE_PREP: return launch_one<T, R, MODE_PREP>(p, st);
-        case MODE_KIN: return launch_one<T, R, MODE_KIN>(p, st);
-        case MODE_SPLITB: return launch_one<T, R, MODE_SPLITB>(p, st);
-        case MODE_LC: return launch_one<T, R, MODE_LC>(p, st);
+        case MODE_APPLY: return launch_one<T, R, MODE_APPLY, HOC>(p, st);
+        case MODE_S1: return launch_one<T, R, MODE_S1, HOC>(p, st);
+        case MODE_S2: return launch_one<T, R, MODE_S2, HOC>(p, st);
+        case MODE_S3: return launch_one<T, R, MODE_S3, HOC>(p, st);
+        case MODE_S4: return launch_one<T, R, MODE_S4, HOC>(p, st);
+        case MODE_IMAG: return launch_one<T, R, MODE_IMAG, HOC>(p, st);
+        case MODE_ENERGY: return launch_one<T, R, MODE_ENERGY, HOC>(p, st);
+        case MODE_PREP: return launch_one<T, R, MODE_PREP, HOC>(p, st);
+        case MODE_KIN: return launch_one<T, R, MODE_KIN, HOC>(p, st);
+        case MODE_SPLITB: return launch_one<T, R, MODE_SPLITB, HOC>(p, st);
+        case MODE_LC: return launch_one<T, R, MODE_LC, HOC>(p, st);
     }
     return cudaErrorInvalidValue;
 }
 
-template <typename T, int R, int MODE>
+template <typename T, int R, int MODE, bool HOC>
 cudaError_t set_attr() {
-    return cudaFuncSetAttribute(stage_kernel<T, R, MODE, rows_per_lane<T>()>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)stage_smem<T, R, MODE>());
+    return cudaFuncSetAttribute(stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)stage_smem<T, R, MODE, HOC>());
 }
-template <typename T, int R>
+template <typename T, int R, bool HOC>
 cudaError_t set_attr_modes() {
     cudaError_t e;
-    if ((e = set_attr<T, R, MODE_APPLY>())) return e;
-    if ((e = set_attr<T, R, MODE_S1>())) return e;
-    if ((e = set_attr<T, R, MODE_S2>())) return e;
-    if ((e = set_attr<T, R, MODE_S3>())) return e;
-    if ((e = set_attr<T, R, MODE_S4>())) return e;
-    if ((e = set_attr<T, R, MODE_IMAG>())) return e;
-    if ((e = set_attr<T, R, MODE_ENERGY>())) return e;
-    if ((e = set_attr<T, R, MODE_PREP>())) return e;
-    if ((e = set_attr<T, R, MODE_KIN>())) return e;
-    if ((e = set_attr<T, R, MODE_SPLITB>())) return e;
-    if ((e = set_attr<T, R, MODE_LC>())) return e;
+    if ((e = set_attr<T, R, MODE_APPLY, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_S1, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_S2, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_S3, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_S4, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_IMAG, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_ENERGY, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_PREP, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_KIN, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_SPLITB, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_LC, HOC>())) return e;
     return cudaSuccess;
 }
 
@@ -590,25 +635,38 @@ cudaError_t set_attr_modes() {
 
 int stage_max_planes() { return KZMAX; }
 
-size_t stage_smem_bytes(int dtype, int radius) {   // largest over the modes (the aux-carrying RK stages)
-    if (dtype == GPE_C128) return radius == 1 ? stage_smem<double, 1, MODE_S2>() : stage_smem<double, 2, MODE_S2>();
-    return radius == 1 ? stage_smem<float, 1, MODE_S2>() : stage_smem<float, 2, MODE_S2>();
+// variant: 1 = 7-point, 2 = 13-point, 3 = 19-point (gpe_internal.h)
+size_t stage_smem_bytes(int dtype, int variant) {   // largest over the modes (the aux-carrying RK stages)
+    if (dtype == GPE_C128)
+        return variant == 1 ? stage_smem<double, 1, MODE_S2, false>()
+                            : (variant == 2 ? stage_smem<double, 2, MODE_S2, false>() : stage_smem<double, 1, MODE_S2, true>());
+    return variant == 1 ? stage_smem<float, 1, MODE_S2, false>()
+                        : (variant == 2 ? stage_smem<float, 2, MODE_S2, false>() : stage_smem<float, 1, MODE_S2, true>());
 }
 
 int kernels_configure() {
     cudaError_t e;
-    if ((e = set_attr_modes<double, 1>())) return (int)e;
-    if ((e = set_attr_modes<double, 2>())) return (int)e;
-    if ((e = set_attr_modes<float, 1>())) return (int)e;
-    if ((e = set_attr_modes<float, 2>())) return (int)e;
+    if ((e = set_attr_modes<double, 1, false>())) return (int)e;
+    if ((e = set_attr_modes<double, 2, false>())) return (int)e;
+    if ((e = set_attr_modes<double, 1, true>())) return (int)e;
+    if ((e = set_attr_modes<float, 1, false>())) return (int)e;
+    if ((e = set_attr_modes<float, 2, false>())) return (int)e;
+    if ((e = set_attr_modes<float, 1, true>())) return (int)e;
     return 0;
 }
 
-int launch_stage(int dtype, int radius, int mode, const StageParams& p, void* stream) {
+template <typename T>
+cudaError_t launch_variant(int variant, int mode, const StageParams& p, cudaStream_t st) {
+    if (variant == 1) return launch_mode<T, 1, false>(mode, p, st);
+    if (variant == 2) return launch_mode<T, 2, false>(mode, p, st);
+    if (variant == 3) return launch_mode<T, 1, true>(mode, p, st);
+    return cudaErrorInvalidValue;
+}
+
+int launch_stage(int dtype, int variant, int mode, const StageParams& p, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     if (p.n_work <= 0) return 0;
-    if (dtype == GPE_C128) return (int)(radius == 1 ? launch_mode<double, 1>(mode, p, st) : launch_mode<double, 2>(mode, p, st));
-    return (int)(radius == 1 ? launch_mode<float, 1>(mode, p, st) : launch_mode<float, 2>(mode, p, st));
+    return (int)(dtype == GPE_C128 ? launch_variant<double>(variant, mode, p, st) : launch_variant<float>(variant, mode, p, st));
 }
 
 }  // namespace gpe

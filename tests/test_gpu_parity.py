@@ -253,3 +253,48 @@ def test_rkck_small_shell_with_ramp(P, stencil, dtype):
     sim.run_rk4(w.dt, 1)
     ref = O.run_rk4(og, pot, w.g, 0.005 + 3 * w.dt, w.dt, 1, ref, stencil)
     assert rel_max(sim.get_psi_host(), ref) < (1e-12 if dtype == "complex128" else 2e-5)
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+def test_19pt_hoc_stencil(P, dtype):
+    """The paper's 19-point higher-order compact Laplacian (PAPER.md:341-343 Eq. B2, isotropic spacing): operator,
+    RK4 with a ramped potential, imaginary time and the energy sums against the oracle; shells with ragged
+    tails (diagonal tiles present and absent) and random masks touching the box faces."""
+    tol = 1e-12 if dtype == "complex128" else 1e-5
+    w = I.small_shell(40, 19, dtype).with_(delta0=14.0, delta1=22.0, t_ramp=0.02)
+    box, pot, act, grid, sim = _make(P, w)
+    og = O.SparseGrid(box, act, 1)
+    psi = I.random_psi(7, act.size).astype(sim.npdtype)
+    for kz in (5, 32):
+        sim.set_planes_per_block(kz)
+        got = sim.apply_H(0.3, _dev(psi, dtype)).cpu().numpy()
+        assert rel_max(got, O.apply_H(og, pot, w.g, 0.3, psi.astype(np.complex128), 19)) < tol
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    sim.time = 0.005
+    sim.run_rk4(w.dt, 3)
+    ref = O.run_rk4(og, pot, w.g, 0.005, w.dt, 3, psi.astype(np.complex128), 19)
+    assert rel_max(sim.get_psi_host(), ref) < tol
+    if dtype == "complex128":
+        e, eo = sim.energy(), O.energy(og, pot, w.g, sim.time, ref, 19)
+        for k in eo:
+            assert abs(e[k] - eo[k]) <= 1e-11 * max(1.0, abs(eo[k])), k
+        sim.set_psi_host(psi)
+        sim.run_imag(1e-3, 4)
+        assert rel_max(sim.get_psi_host(), O.run_imag(og, pot, w.g, sim.time, 1e-3, 4, psi, 19)) < tol
+        sim.set_psi_host(psi)
+        sim.run_imag_split(1e-3, 3)
+        assert rel_max(sim.get_psi_host(), O.run_imag_split(og, pot, w.g, sim.time, 1e-3, 3, psi, 19)) < tol
+
+
+@pytest.mark.parametrize("dims,p,seed", [((9, 7, 11), 0.4, 3), ((17, 16, 40), 0.15, 4), ((6, 6, 6), 1.1, 6), ((19, 21, 37), 0.6, 8)])
+def test_19pt_random_masks(P, dims, p, seed):
+    nx, ny, nz = dims
+    w = I.Workload(name="rnd", nx=nx, ny=ny, nz=nz, h=0.3, kind=I.DRESSED, ax=1.0, ay=0.7, az=1.2, delta0=2.0,
+                   delta1=2.0, omega=1.5, stencil=19, g=3.0)
+    act = I.random_mask_lin(seed, nx, ny, nz, p)
+    box, pot, act, grid, sim = _make(P, w, active=act)
+    og = O.SparseGrid(box, act, 1)
+    psi = I.random_psi(seed + 100, act.size)
+    got = sim.apply_H(0.1, _dev(psi, "complex128")).cpu().numpy()
+    assert rel_max(got, O.apply_H(og, pot, w.g, 0.1, psi, 19)) < 1e-12

@@ -298,3 +298,21 @@ def test_19pt_random_masks(P, dims, p, seed):
     psi = I.random_psi(seed + 100, act.size)
     got = sim.apply_H(0.1, _dev(psi, "complex128")).cpu().numpy()
     assert rel_max(got, O.apply_H(og, pot, w.g, 0.1, psi, 19)) < 1e-12
+
+
+@pytest.mark.parametrize("dtype,stencil", [("complex128", 13), ("complex64", 13), ("complex128", 19)])
+def test_small_shell_1000_steps(P, dtype, stencil):
+    """The north_star's long-run bound on a shell (ragged tiles, ramped potential): max relative error 1e-9 after
+    1000 RK4 steps in complex128, 1e-3 in complex64 (19-point: 200 steps)."""
+    w = I.small_shell(40, stencil, dtype).with_(delta0=14.0, delta1=16.0, t_ramp=0.5)
+    box, pot, act, grid, sim = _make(P, w)
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    nsteps = 200 if stencil == 19 else 1000          # the NumPy oracle (no C restatement of the 19-point stencil)
+    sim.run_rk4(w.dt, nsteps)
+    if stencil == 19:
+        og = O.SparseGrid(box, act, 1)
+        ref = O.run_rk4(og, pot, w.g, 0.0, w.dt, nsteps, psi.astype(np.complex128), 19)
+    else:
+        ref = CO.COracle(box, pot, act, stencil).run_rk4(w.g, 0.0, w.dt, 1000, psi.astype(np.complex128))
+    assert rel_max(sim.get_psi_host(), ref) < TOL_STEPS[dtype]

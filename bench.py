@@ -131,7 +131,7 @@ def oracle_sample(w, target_points=3_000_000):
     """Bounded sample of the workload for the CPU oracle: the active points of a slab ix in [lo, hi) of the
     same box and potential (a truncated shell; psi = 0 outside it), about `target_points` points."""
     from oracle import gpe_oracle as O
-    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center)
+    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center, w.hy, w.hz)
     pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
     plane = w.ny * w.nz
     mid = w.nx // 2

@@ -59,6 +59,12 @@ class Workload:
     psi0: str = "shell"       # gaussian | constant | shell | blob
     center: tuple = (0.0, 0.0, 0.0)
     note: str = ""
+    hy: float = 0.0           # step sizes along y, z; <= 0: same as h (anisotropic grids, App. B)
+    hz: float = 0.0
+
+    @property
+    def spacing(self):
+        return (self.h, self.hy if self.hy > 0 else self.h, self.hz if self.hz > 0 else self.h)
 
     def with_(self, **kw) -> "Workload":
         return replace(self, **kw)
@@ -182,8 +188,8 @@ def _coords_of(w: Workload, lin: np.ndarray):
     iy = (lin // w.nz) % w.ny
     ix = lin // (w.nz * w.ny)
     x = (ix.astype(np.float64) - 0.5 * (w.nx - 1)) * w.h + w.center[0]
-    y = (iy.astype(np.float64) - 0.5 * (w.ny - 1)) * w.h + w.center[1]
-    z = (iz.astype(np.float64) - 0.5 * (w.nz - 1)) * w.h + w.center[2]
+    y = (iy.astype(np.float64) - 0.5 * (w.ny - 1)) * w.spacing[1] + w.center[1]
+    z = (iz.astype(np.float64) - 0.5 * (w.nz - 1)) * w.spacing[2] + w.center[2]
     return x, y, z
 
 
@@ -229,7 +235,7 @@ def make_psi0(w: Workload, active_idx: np.ndarray, n_target: float = 1.0) -> np.
     else:
         raise ValueError(w.psi0)
     psi = amp * np.exp(1j * phi)
-    nrm = w.h ** 3 * float(np.sum(np.abs(psi) ** 2))
+    nrm = w.spacing[0] * w.spacing[1] * w.spacing[2] * float(np.sum(np.abs(psi) ** 2))
     psi *= math.sqrt(n_target / nrm)
     return psi.astype(np.complex128)
 

@@ -59,8 +59,12 @@ typedef struct gpe_sim gpe_sim;   /* opaque: one wavefunction evolving on a grid
 typedef struct {
     int32_t nx, ny, nz; /* box size in points, each >= 1 */
     int32_t reserved;   /* must be 0 */
-    double h;           /* grid spacing, > 0 */
+    double h;           /* grid spacing (along x when hy / hz are given), > 0 */
     double center[3];   /* coordinate of the box centre */
+    double hy, hz;      /* grid spacing along y and z for anisotropic grids d_x != d_y != d_z (PAPER.md:333-343
+                           App. B: every second difference carries its own 1/d_i^2, the 19-point cross terms
+                           (d_i^2 + d_j^2)/12); <= 0 means "same as h".  Sums that stand for integrals use the
+                           volume element h hy hz. */
 } gpe_box;
 
 typedef struct {

@@ -21,7 +21,7 @@ class _Problem(C.Structure):
                 ("h", C.c_double), ("cx", C.c_double), ("cy", C.c_double), ("cz", C.c_double),
                 ("ax", C.c_double), ("ay", C.c_double), ("az", C.c_double),
                 ("delta0", C.c_double), ("delta1", C.c_double), ("t_ramp", C.c_double),
-                ("omega", C.c_double)]
+                ("omega", C.c_double), ("hy", C.c_double), ("hz", C.c_double)]
 
 
 def build(force: bool = False) -> str:
@@ -54,7 +54,7 @@ class COracle:
         self.lib = _load()
         self.prob = _Problem(box.nx, box.ny, box.nz, pot.kind, box.h, box.center[0], box.center[1],
                              box.center[2], pot.ax, pot.ay, pot.az, pot.delta0, pot.delta1,
-                             pot.t_ramp, pot.omega)
+                             pot.t_ramp, pot.omega, box.spacing[1], box.spacing[2])
         self.active = np.ascontiguousarray(active, dtype=np.int64)
         self.n = self.active.size
         self.R = {7: 1, 13: 2}[stencil]

@@ -52,6 +52,18 @@ class Box:
     nz: int
     h: float
     center: tuple = (0.0, 0.0, 0.0)
+    hy: float = 0.0          # step sizes along y and z; <= 0 means "same as h" (App. B:
+    hz: float = 0.0          # anisotropic grids d_x != d_y != d_z)
+
+    @property
+    def spacing(self):
+        return (self.h, self.hy if self.hy > 0 else self.h, self.hz if self.hz > 0 else self.h)
+
+    @property
+    def cell(self):
+        """Volume element d_x d_y d_z of the sums that stand for integrals (Eq. 3)."""
+        d = self.spacing
+        return d[0] * d[1] * d[2]
 
 
 @dataclass
@@ -103,8 +115,8 @@ def potential_from_u(pot: Potential, u, delta):
 def mask_potential_plane(box: Box, pot: Potential, mask_mode: int, ix: int) -> np.ndarray:
     """V_mask on the (ny, nz) plane ix (R13 for the UNION closed form)."""
     x = coords(box.nx, box.h, box.center[0])[ix]
-    y = coords(box.ny, box.h, box.center[1])[:, None]
-    z = coords(box.nz, box.h, box.center[2])[None, :]
+    y = coords(box.ny, box.spacing[1], box.center[1])[:, None]
+    z = coords(box.nz, box.spacing[2], box.center[2])[None, :]
     u = quad_form(pot, x, y, z)
     if pot.kind == HARMONIC:
         return u
@@ -147,8 +159,8 @@ def potential_at(box: Box, pot: Potential, lin: np.ndarray, t: float) -> np.ndar
     """V(r_p, t) on the given points (evaluated at the stage time, Eq. 9)."""
     ix, iy, iz = unravel(box, lin)
     x = coords(box.nx, box.h, box.center[0])[ix]
-    y = coords(box.ny, box.h, box.center[1])[iy]
-    z = coords(box.nz, box.h, box.center[2])[iz]
+    y = coords(box.ny, box.spacing[1], box.center[1])[iy]
+    z = coords(box.nz, box.spacing[2], box.center[2])[iz]
     u = quad_form(pot, x, y, z)
     return potential_from_u(pot, u, delta_of_t(pot, t))
 
@@ -206,30 +218,31 @@ def neighbour_lookup(grid: SparseGrid, off) -> np.ndarray:
 
 
 def apply_T19(grid: SparseGrid, psi: np.ndarray) -> np.ndarray:
-    """T psi = -1/2 lap_19 psi with the 19-point higher-order compact Laplacian of PAPER.md:341-343 Eq. B2 for
-    dx = dy = dz = h:  lap_19 = lap_7 + (h^2/6) (dxx dyy + dxx dzz + dyy dzz),  d_ii = [1,-2,1]/h^2, written out
-    term by term as in Eq. B2 (products of second differences), psi = 0 outside M."""
+    """T psi = -1/2 lap_19 psi with the 19-point higher-order compact Laplacian of PAPER.md:341-343 Eq. B2,
+      lap_19 = lap_7 + 1/12 [ (dx^2+dy^2) dxx dyy + (dx^2+dz^2) dxx dzz + (dy^2+dz^2) dyy dzz ],  d_ii = [1,-2,1]/d_i^2,
+    written out term by term as printed (products of second differences), psi = 0 outside M."""
     psi = np.asarray(psi, dtype=np.complex128)
-    h2 = grid.box.h * grid.box.h
+    dsq = [d * d for d in grid.box.spacing]
     ext = np.concatenate([psi, np.zeros(1, np.complex128)])   # index -1 -> 0
     d2 = (1.0, -2.0, 1.0)
 
     def term(wx, wy, wz):
-        """sum over offsets of wx[dx] wy[dy] wz[dz] psi(p + (dx,dy,dz)); w = None is the identity [0,1,0]."""
+        """sum over offsets of wx[dx] wy[dy] wz[dz] psi(p + (dx,dy,dz)); w = False is the identity [0,1,0]."""
         out = np.zeros_like(psi)
         for dx in (-1, 0, 1):
             for dy in (-1, 0, 1):
                 for dz in (-1, 0, 1):
                     c = 1.0
-                    for wgt, d in ((wx, dx), (wy, dy), (wz, dz)):
-                        c *= (d2[d + 1] / h2) if wgt else (1.0 if d == 0 else 0.0)
+                    for axis, (wgt, d) in enumerate(((wx, dx), (wy, dy), (wz, dz))):
+                        c *= (d2[d + 1] / dsq[axis]) if wgt else (1.0 if d == 0 else 0.0)
                     if c != 0.0:
                         out = out + c * ext[neighbour_lookup(grid, (dx, dy, dz))]
         return out
 
     lap7 = term(True, False, False) + term(False, True, False) + term(False, False, True)
-    cross = term(True, True, False) + term(True, False, True) + term(False, True, True)
-    return -0.5 * (lap7 + (1.0 / 12.0) * (2.0 * h2) * cross)
+    cross = ((dsq[0] + dsq[1]) * term(True, True, False) + (dsq[0] + dsq[2]) * term(True, False, True)
+             + (dsq[1] + dsq[2]) * term(False, True, True))
+    return -0.5 * (lap7 + (1.0 / 12.0) * cross)
 
 
 def apply_T(grid: SparseGrid, psi: np.ndarray, stencil: int) -> np.ndarray:
@@ -244,12 +257,14 @@ def apply_T(grid: SparseGrid, psi: np.ndarray, stencil: int) -> np.ndarray:
     R = len(w) - 1
     assert R <= grid.radius
     psi = np.asarray(psi, dtype=np.complex128)
-    lap = (3.0 * w[0]) * psi
     ext = np.concatenate([psi, np.zeros(1, np.complex128)])  # index -1 -> 0
-    for axis in range(3):
+    lap = np.zeros_like(psi)
+    for axis in range(3):                                    # Eq. B1: each axis with its own step size d_i
+        d = w[0] * psi
         for s in range(1, R + 1):
-            lap = lap + w[s] * (ext[grid.nbr[(axis, -s)]] + ext[grid.nbr[(axis, s)]])
-    return (-0.5 / (grid.box.h * grid.box.h)) * lap
+            d = d + w[s] * (ext[grid.nbr[(axis, -s)]] + ext[grid.nbr[(axis, s)]])
+        lap = lap + d / (grid.box.spacing[axis] ** 2)
+    return -0.5 * lap
 
 
 def apply_H(grid: SparseGrid, pot: Potential, g: float, t: float, psi: np.ndarray,
@@ -340,7 +355,7 @@ def _sum(x) -> float:
 
 def norm(grid: SparseGrid, psi) -> float:
     """h^3 sum |psi|^2  (Eq. 3)."""
-    return grid.box.h ** 3 * _sum(psi.real ** 2 + psi.imag ** 2)
+    return grid.box.cell * _sum(psi.real ** 2 + psi.imag ** 2)
 
 
 def imag_step(grid, pot, g, t, dt, psi, stencil, n_target=1.0):
@@ -407,7 +422,7 @@ def energy(grid, pot, g, t, psi, stencil) -> dict:
     inter = h^3 (g/2) sum |psi|^4; total = kin+pot+inter;
     mu = h^3 sum Re(conj(psi) H psi) / norm = (kin + pot + 2 inter)/norm (Eq. 1).
     """
-    h3 = grid.box.h ** 3
+    h3 = grid.box.cell
     tp = apply_T(grid, psi, stencil)
     v = potential_at(grid.box, pot, grid.active, t)
     a2 = psi.real ** 2 + psi.imag ** 2
@@ -428,8 +443,10 @@ def dense_apply_T(box: Box, mask: np.ndarray, psi_dense: np.ndarray, stencil: in
     w = STENCIL_WEIGHTS[stencil]
     R = len(w) - 1
     p = np.where(mask, psi_dense, 0.0).astype(np.complex128)
-    lap = 3.0 * w[0] * p
+    lap = np.zeros_like(p)
     for axis in range(3):
+        inv = 1.0 / box.spacing[axis] ** 2
+        lap += (w[0] * inv) * p
         for s in range(1, R + 1):
             for sg in (-s, s):
                 sh = np.zeros_like(p)
@@ -442,8 +459,8 @@ def dense_apply_T(box: Box, mask: np.ndarray, psi_dense: np.ndarray, stencil: in
                     src[axis] = slice(None, sg)
                     dst[axis] = slice(-sg, None)
                 sh[tuple(dst)] = p[tuple(src)]
-                lap += w[s] * sh
-    return np.where(mask, (-0.5 / (box.h * box.h)) * lap, 0.0)
+                lap += (w[s] * inv) * sh
+    return np.where(mask, -0.5 * lap, 0.0)
 
 
 # --------------------------------------------------------------------------

@@ -30,6 +30,7 @@ typedef struct {
     double h, cx, cy, cz;
     double ax, ay, az;
     double delta0, delta1, t_ramp, omega;
+    double hy, hz;              /* step sizes along y, z (App. B Eq. B1); the wrapper passes h when isotropic */
 } orc_problem;
 
 int orc_num_threads(void) {
@@ -82,8 +83,8 @@ static double delta_of_t(const orc_problem* p, double t) {
 static double potential(const orc_problem* p, int64_t L, double delta) {
     int64_t ix = L / ((int64_t)p->ny * p->nz), iy = (L / p->nz) % p->ny, iz = L % p->nz;
     double x = ((double)ix - 0.5 * (p->nx - 1)) * p->h + p->cx;
-    double y = ((double)iy - 0.5 * (p->ny - 1)) * p->h + p->cy;
-    double z = ((double)iz - 0.5 * (p->nz - 1)) * p->h + p->cz;
+    double y = ((double)iy - 0.5 * (p->ny - 1)) * p->hy + p->cy;
+    double z = ((double)iz - 0.5 * (p->nz - 1)) * p->hz + p->cz;
     double s = p->ax * (x * x) + p->ay * (y * y) + p->az * (z * z);
     double u = 0.5 * s;
     if (p->kind == 0) return u;
@@ -98,21 +99,24 @@ void orc_apply_H(const orc_problem* p, const int64_t* active, const int64_t* nbr
     const double w13[3] = {-5.0 / 2.0, 4.0 / 3.0, -1.0 / 12.0};
     const double* w = (R == 1) ? w7 : w13;
     const double delta = delta_of_t(p, t);
-    const double pref = -0.5 / (p->h * p->h);
+    const double inv[3] = {1.0 / (p->h * p->h), 1.0 / (p->hy * p->hy), 1.0 / (p->hz * p->hz)};   /* Eq. B1: 1/d_i^2 */
 #pragma omp parallel for schedule(static)
     for (int64_t k = 0; k < n; ++k) {
-        cplx lap = (3.0 * w[0]) * psi[k];
-        for (int axis = 0; axis < 3; ++axis)
+        cplx lap = 0.0;
+        for (int axis = 0; axis < 3; ++axis) {
+            cplx d2 = w[0] * psi[k];
             for (int s = 1; s <= R; ++s) {
                 int64_t m = nbr[k * 6 * R + axis * 2 * R + (R - s)];       /* -s */
                 int64_t q = nbr[k * 6 * R + axis * 2 * R + (R + s - 1)];   /* +s */
                 cplx a = (m >= 0) ? psi[m] : 0.0;
                 cplx b = (q >= 0) ? psi[q] : 0.0;
-                lap += w[s] * (a + b);
+                d2 += w[s] * (a + b);
             }
+            lap += inv[axis] * d2;
+        }
         double v = potential(p, active[k], delta);
         double a2 = creal(psi[k]) * creal(psi[k]) + cimag(psi[k]) * cimag(psi[k]);
-        out[k] = pref * lap + (v + g * a2) * psi[k];
+        out[k] = -0.5 * lap + (v + g * a2) * psi[k];
     }
 }
 
@@ -149,7 +153,7 @@ static double norm_sum(int64_t n, const cplx* psi) {
 }
 
 double orc_norm(const orc_problem* p, int64_t n, const cplx* psi) {
-    return p->h * p->h * p->h * norm_sum(n, psi);
+    return p->h * p->hy * p->hz * norm_sum(n, psi);
 }
 
 /* nsteps normalised forward-Euler imaginary-time steps, V frozen at time t; work holds n values */
@@ -182,7 +186,7 @@ void orc_energy(const orc_problem* p, const int64_t* active, const int64_t* nbr,
         in4 += (long double)(a2 * a2);
         nn += (long double)a2;
     }
-    double h3 = p->h * p->h * p->h;
+    double h3 = p->h * p->hy * p->hz;
     out[0] = h3 * (double)kin;
     out[1] = h3 * (double)po;
     out[2] = h3 * 0.5 * g * (double)in4;

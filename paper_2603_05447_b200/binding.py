@@ -30,7 +30,7 @@ class GpeError(RuntimeError):
 
 class Box(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("reserved", C.c_int32),
-                ("h", C.c_double), ("center", C.c_double * 3)]
+                ("h", C.c_double), ("center", C.c_double * 3), ("hy", C.c_double), ("hz", C.c_double)]
 
 
 class Potential(C.Structure):
@@ -95,8 +95,8 @@ class Grid:
 
     def __init__(self, nx, ny, nz, h, kind=HARMONIC, ax=1.0, ay=1.0, az=1.0, delta0=0.0, delta1=0.0,
                  t_ramp=0.0, omega=0.0, mask_mode=MASK_AT_DELTA0, v_cut=math.inf, halo_width=2,
-                 center=(0.0, 0.0, 0.0), active=None):
-        self.box = Box(nx, ny, nz, 0, h, (C.c_double * 3)(*center))
+                 center=(0.0, 0.0, 0.0), active=None, hy=0.0, hz=0.0):
+        self.box = Box(nx, ny, nz, 0, h, (C.c_double * 3)(*center), hy, hz)
         self.pot = Potential(kind, mask_mode, ax, ay, az, delta0, delta1, t_ramp, omega)
         self._h = C.c_void_p()
         L = lib()
@@ -111,7 +111,8 @@ class Grid:
     @classmethod
     def from_workload(cls, w, active=None):
         return cls(w.nx, w.ny, w.nz, w.h, w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega,
-                   w.mask_mode, w.v_cut, w.halo_width, w.center, active=active)
+                   w.mask_mode, w.v_cut, w.halo_width, w.center, active=active, hy=getattr(w, "hy", 0.0),
+                   hz=getattr(w, "hz", 0.0))
 
     def close(self):
         if self._h:

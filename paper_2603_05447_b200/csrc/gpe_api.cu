@@ -72,6 +72,8 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e__ != 0) return cuda_fail((cudaError_t)e__, #call);       \
     } while (0)
 
+double cell_volume(const gpe_box& b) { return b.h * (b.hy > 0.0 ? b.hy : b.h) * (b.hz > 0.0 ? b.hz : b.h); }
+
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 size_t buf_bytes(int64_t n, int dtype) { return align_up((size_t)(n > 0 ? n : 1) * (dtype == GPE_C128 ? 16 : 8), 256); }
@@ -81,7 +83,8 @@ PotDev pot_dev(const gpe_sim* s, double t) {
     PotDev p;
     p.kind = h.pot.kind;
     p.nx = h.box.nx; p.ny = h.box.ny; p.nz = h.box.nz;
-    p.h = h.box.h; p.cx = h.box.center[0]; p.cy = h.box.center[1]; p.cz = h.box.center[2];
+    p.h = h.box.h; p.hy = h.box.hy > 0.0 ? h.box.hy : h.box.h; p.hz = h.box.hz > 0.0 ? h.box.hz : h.box.h;
+    p.cx = h.box.center[0]; p.cy = h.box.center[1]; p.cz = h.box.center[2];
     p.ax = h.pot.ax; p.ay = h.pot.ay; p.az = h.pot.az;
     p.delta = delta_of_t(h.pot, t);
     p.omega = h.pot.omega;
@@ -189,16 +192,27 @@ StageParams base_params(const gpe_sim* s, double t) {
     p.partials = s->d_partials;
     p.scale_in = s->d_sums + NACC;
     const GridHost& h = s->grid->h;
-    const double ih2 = -0.5 / (h.box.h * h.box.h);
-    p.kw[0] = ih2 * 3.0 * (s->radius == 1 ? -2.0 : -2.5);
-    p.kw[1] = ih2 * (s->radius == 1 ? 1.0 : 4.0 / 3.0);
-    p.kw[2] = s->radius == 1 ? 0.0 : ih2 * (-1.0 / 12.0);
-    if (s->hoc) {   // PAPER.md:343 Eq. B2 with dx = dy = dz = h: centre -4, faces 1/3, edges 1/6 (over h^2)
-        p.kw[0] = ih2 * -4.0;
-        p.kw[1] = ih2 * (1.0 / 3.0);
-        p.kw[2] = ih2 * (1.0 / 6.0);
+    // Eq. B1: each axis with its own 1/d_a^2; star weights c_0, c_1, c_2 (R5); all times -1/2
+    const double c0 = s->radius == 1 ? -2.0 : -2.5, c1 = s->radius == 1 ? 1.0 : 4.0 / 3.0, c2 = s->radius == 1 ? 0.0 : -1.0 / 12.0;
+    const double ia[3] = {1.0 / (p.pot.h * p.pot.h), 1.0 / (p.pot.hy * p.pot.hy), 1.0 / (p.pot.hz * p.pot.hz)};
+    for (int a = 0; a < 3; ++a) { p.kw[a][0] = 0.0; p.kw[a][1] = -0.5 * c1 * ia[a]; p.kw[a][2] = -0.5 * c2 * ia[a]; }
+    p.kw[0][0] = -0.5 * c0 * (ia[0] + ia[1] + ia[2]);
+    p.ke[0] = p.ke[1] = p.ke[2] = 0.0;
+    if (s->hoc) {
+        // Eq. B2: lap_19 = lap_7 + sum_pairs (d_i^2 + d_j^2)/12 d_ii d_jj; (d_i^2 + d_j^2)/(d_i^2 d_j^2) = 1/d_i^2 + 1/d_j^2,
+        // so the pair weight is c_ij = (1/d_i^2 + 1/d_j^2)/12: edges c_ij, faces 1/d_i^2 - 2 (c_ij + c_ik),
+        // centre -2 sum 1/d_i^2 + 4 sum c_ij  (isotropic: -4, 1/3, 1/6 over h^2)
+        const double cxy = (ia[0] + ia[1]) / 12.0, cxz = (ia[0] + ia[2]) / 12.0, cyz = (ia[1] + ia[2]) / 12.0;
+        p.kw[0][0] = -0.5 * (-2.0 * (ia[0] + ia[1] + ia[2]) + 4.0 * (cxy + cxz + cyz));
+        p.kw[0][1] = -0.5 * (ia[0] - 2.0 * (cxy + cxz));
+        p.kw[1][1] = -0.5 * (ia[1] - 2.0 * (cxy + cyz));
+        p.kw[2][1] = -0.5 * (ia[2] - 2.0 * (cxz + cyz));
+        p.ke[0] = -0.5 * cxy; p.ke[1] = -0.5 * cxz; p.ke[2] = -0.5 * cyz;
     }
-    for (int k = 0; k < 3; ++k) p.kwf[k] = (float)p.kw[k];
+    for (int a = 0; a < 3; ++a) {
+        for (int k = 0; k < 3; ++k) p.kwf[a][k] = (float)p.kw[a][k];
+        p.kef[a] = (float)p.ke[a];
+    }
     p.xc = 0.5 * (double)(h.box.nx - 1);
     p.yc = 0.5 * (double)(h.box.ny - 1);
     p.zc = 0.5 * (double)(h.box.nz - 1);
@@ -482,7 +496,7 @@ int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream) {
     if (!src || !dst || src == dst) return fail(GPE_ERR_INVALID_ARG, "null or identical simulations");
     if (src->dtype != dst->dtype) return fail(GPE_ERR_INVALID_ARG, "source and destination precisions differ");
     const gpe_box &a = src->grid->h.box, &b = dst->grid->h.box;
-    if (a.nx != b.nx || a.ny != b.ny || a.nz != b.nz || a.h != b.h || a.center[0] != b.center[0] ||
+    if (a.nx != b.nx || a.ny != b.ny || a.nz != b.nz || a.h != b.h || a.hy != b.hy || a.hz != b.hz || a.center[0] != b.center[0] ||
         a.center[1] != b.center[1] || a.center[2] != b.center[2])
         return fail(GPE_ERR_INVALID_ARG, "the two grids must be post-selected from the same bounding box");
     dst->t = src->t;
@@ -619,7 +633,7 @@ int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
     if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
     if (s->n == 0 || nsteps == 0) return GPE_OK;
-    const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;
+    const double h3 = cell_volume(s->grid->h.box);
     for (int64_t n = 0; n < nsteps; ++n) {
         int rc = stage(s, MODE_IMAG, s->t, dt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
         if (rc) return rc;
@@ -640,7 +654,7 @@ int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
     if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
     if (s->n == 0 || nsteps == 0) return GPE_OK;
-    const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;
+    const double h3 = cell_volume(s->grid->h.box);
     const double hdt = 0.5 * dt;
     for (int64_t n = 0; n < nsteps; ++n) {
         // A holds the un-normalised state of the previous iteration; its scale sits in d_sums[NACC]
@@ -662,7 +676,7 @@ int gpe_imag_split_step(gpe_sim* s, double dt, void* stream) { return gpe_run_im
 
 int gpe_norm(gpe_sim* s, double* out_host, void* stream) {
     if (!s || !out_host) return fail(GPE_ERR_INVALID_ARG, "null argument");
-    const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;
+    const double h3 = cell_volume(s->grid->h.box);
     if (s->n == 0) { *out_host = 0.0; return GPE_OK; }
     KL(launch_norm_partials(s->dtype, s->buf[0], s->n, s->d_partials, stream));
     KL(launch_finalize(s->d_partials, norm_blocks(s->n), s->d_sums, nullptr, s->n_target, h3, stream));
@@ -678,7 +692,7 @@ int gpe_norm(gpe_sim* s, double* out_host, void* stream) {
 
 int gpe_energy(gpe_sim* s, gpe_energy_out* o, void* stream) {
     if (!s || !o) return fail(GPE_ERR_INVALID_ARG, "null argument");
-    const double h3 = s->grid->h.box.h * s->grid->h.box.h * s->grid->h.box.h;
+    const double h3 = cell_volume(s->grid->h.box);
     if (s->n == 0) return fail(GPE_ERR_STATE, "empty grid has no energy");
     int rc = stage(s, MODE_ENERGY, s->t, 0.0, s->buf[0], nullptr, nullptr, nullptr, stream);
     if (rc) return rc;

@@ -78,7 +78,8 @@ static_assert(sizeof(WorkRec) == 192, "WorkRec layout");
 struct PotDev {
     int32_t kind;
     int32_t nx, ny, nz;
-    double h, cx, cy, cz;
+    double h, cx, cy, cz;   // h = spacing along x
+    double hy, hz;          // spacing along y, z (= h on isotropic grids)
     double ax, ay, az;
     double delta;   // Delta at the stage time (host-computed, R16)
     double omega;
@@ -112,9 +113,13 @@ struct StageParams {
     double g;
     double ca;             // stage coefficient (dt/2, dt, dt/6, or dt of the imaginary step)
     // host-precomputed constants (read from the parameter bank, no registers):
-    double kw[3];          // -1/(2h^2) * {3 c_0, c_1, c_2} of the star stencils; 19-point: * {centre, face, edge} weights
-    float kwf[3];          // the same in fp32 (complex64 state)
-    float padf;
+    // stencil weights times -1/2, per axis a = x, y, z with its own 1/d_a^2 (PAPER.md:337-343 Eq. B1-B2):
+    // kw[a][s] = weight of the neighbours s steps along a (s = 1, 2; 19-point: the face weight at s = 1);
+    // kw[0][0] = the centre weight (all axes together); ke[] = 19-point edge weights xy, xz, yz
+    double kw[3][3];
+    double ke[3];
+    float kwf[3][3];       // the same in fp32 (complex64 state)
+    float kef[3];
     double xc, yc, zc;     // 0.5 (n-1) per axis: coordinate = (i - xc) h + cx
     double hax, hay, haz;  // 0.5 a_x, 0.5 a_y, 0.5 a_z
     double om2;            // Omega^2

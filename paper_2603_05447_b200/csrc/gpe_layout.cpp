@@ -50,6 +50,7 @@ inline double mask_potential(const gpe_potential& p, double sxy, double szz) {
 int check_box(const gpe_box& b, std::string* err) {
     if (b.nx < 1 || b.ny < 1 || b.nz < 1) { *err = "box dimensions must be >= 1"; return GPE_ERR_INVALID_ARG; }
     if (!(b.h > 0.0) || !std::isfinite(b.h)) { *err = "h must be finite and > 0"; return GPE_ERR_INVALID_ARG; }
+    if (!std::isfinite(b.hy) || !std::isfinite(b.hz)) { *err = "hy and hz must be finite (<= 0: same as h)"; return GPE_ERR_INVALID_ARG; }
     if (b.reserved != 0) { *err = "gpe_box.reserved must be 0"; return GPE_ERR_INVALID_ARG; }
     long double npts = (long double)b.nx * b.ny * b.nz;
     if (npts > 4.0e18L) { *err = "box has more than 2^62 points"; return GPE_ERR_INVALID_ARG; }
@@ -187,7 +188,7 @@ int build_layout_from_potential(const gpe_box& box, const gpe_potential& pot, do
 
     // z-dependent term computed once; one tile-row (tx x-planes) per parallel task
     std::vector<double> zz(box.nz);
-    for (int iz = 0; iz < box.nz; ++iz) { double z = coord(iz, box.nz, box.h, box.center[2]); zz[iz] = pot.az * (z * z); }
+    for (int iz = 0; iz < box.nz; ++iz) { double z = coord(iz, box.nz, box.hz > 0.0 ? box.hz : box.h, box.center[2]); zz[iz] = pot.az * (z * z); }
 
     std::vector<std::vector<TileTmp>> rows(ntx);
     bool oom = false;
@@ -204,7 +205,7 @@ int build_layout_from_potential(const gpe_box& box, const gpe_potential& pot, do
                 if (ix >= box.nx) break;
                 double x = coord(ix, box.nx, box.h, box.center[0]);
                 for (int iy = 0; iy < box.ny; ++iy) {
-                    double y = coord(iy, box.ny, box.h, box.center[1]);
+                    double y = coord(iy, box.ny, box.hy > 0.0 ? box.hy : box.h, box.center[1]);
                     const double sxy = pot.ax * (x * x) + pot.ay * (y * y);
                     const int j = iy / ty;
                     const uint64_t bit = 1ull << (lx * ty + iy % ty);

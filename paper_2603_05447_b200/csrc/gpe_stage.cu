@@ -129,10 +129,14 @@ template <typename T, int R, bool AUX, bool HOC = false> struct Geo {
 
 template <typename T> struct KW;   // stencil weights of the right type straight from the parameter block
 template <> struct KW<double> {
-    static __device__ __forceinline__ double w(const StageParams& p, int s) { return p.kw[s]; }
+    static __device__ __forceinline__ double w(const StageParams& p, int axis, int s) { return p.kw[axis][s]; }
+    static __device__ __forceinline__ double c(const StageParams& p) { return p.kw[0][0]; }
+    static __device__ __forceinline__ double e(const StageParams& p, int pair) { return p.ke[pair]; }
 };
 template <> struct KW<float> {
-    static __device__ __forceinline__ float w(const StageParams& p, int s) { return p.kwf[s]; }
+    static __device__ __forceinline__ float w(const StageParams& p, int axis, int s) { return p.kwf[axis][s]; }
+    static __device__ __forceinline__ float c(const StageParams& p) { return p.kwf[0][0]; }
+    static __device__ __forceinline__ float e(const StageParams& p, int pair) { return p.kef[pair]; }
 };
 
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
@@ -239,7 +243,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
     // potential: u = qxy[e] + qz(plane); qxy = 1/2 (ax x^2 + ay y^2) of the patch points
     double qxy[PR];
     {
-        const double y = ((double)(w->iy0 + ly) - p.yc) * p.pot.h + p.pot.cy;
+        const double y = ((double)(w->iy0 + ly) - p.yc) * p.pot.hy + p.pot.cy;
         const double qy = p.hay * (y * y);
 #pragma unroll
         for (int e = 0; e < PR; ++e) {
@@ -314,9 +318,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
 #pragma unroll
         for (int e = 0; e < PR; ++e) { SP[s][e] = mk<T>((T)0, (T)0); SA[s][e] = mk<T>((T)0, (T)0); }
     double acc[NACC] = {0.0, 0.0, 0.0, 0.0};
-    C FPV[PR];                                             // 19-point: in-plane face sum of the previous plane
+    C GPV[PR];                                             // 19-point: edge contribution G of the previous plane
 #pragma unroll
-    for (int e = 0; e < PR; ++e) FPV[e] = mk<T>((T)0, (T)0);
+    for (int e = 0; e < PR; ++e) GPV[e] = mk<T>((T)0, (T)0);
 
     // ---- prologue: planes 0 .. PF-1 in flight ----------------------------------------------------------------
 #pragma unroll
@@ -376,7 +380,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
         //      interleaved) are issued here and overlap the shared-memory latency of psi(k) --------------------
         double vpot[PR];
         if (cany && MODE != MODE_KIN) {
-            const double zc = ((double)(kstart + ic) - p.zc) * p.pot.h + p.pot.cz;
+            const double zc = ((double)(kstart + ic) - p.zc) * p.pot.hz + p.pot.cz;
             const double qz = p.haz * (zc * zc) - p.delta_eff;
 #pragma unroll
             for (int e = 0; e < PR; ++e) vpot[e] = qxy[e] + qz;
@@ -385,8 +389,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 for (int e = 0; e < PR; ++e) vpot[e] = fast_sqrt(fma(vpot[e], vpot[e], p.om2)) - p.pot.omega;
             }
         }
-        // ---- 19-point: in-plane face sum F and diagonal sum E of the patch points in plane k -------------------
-        C F[PR], E[PR];
+        // ---- 19-point: in-plane face sums (x and y) and diagonal sum E of the patch points in plane k; G = the
+        //      part of plane k that the neighbouring planes see as their xz / yz edge neighbours ----------------
+        C Fx[PR], Fy[PR], E[PR], G[PR];
         if (HOC && MODE != MODE_PREP) {
             C Lc[4], Rc[4], Mc[4];                              // columns ly-1, ly+1, ly of rows -1 .. 2 of the patch
 #pragma unroll
@@ -397,22 +402,24 @@ stage_kernel(const __grid_constant__ StageParams p) {
             }
 #pragma unroll
             for (int a = 0; a < PR; ++a) {
-                F[a] = mk<T>((Mc[a].x + Mc[a + 2].x) + (Lc[a + 1].x + Rc[a + 1].x), (Mc[a].y + Mc[a + 2].y) + (Lc[a + 1].y + Rc[a + 1].y));
+                Fx[a] = mk<T>(Mc[a].x + Mc[a + 2].x, Mc[a].y + Mc[a + 2].y);
+                Fy[a] = mk<T>(Lc[a + 1].x + Rc[a + 1].x, Lc[a + 1].y + Rc[a + 1].y);
                 E[a] = mk<T>((Lc[a].x + Rc[a].x) + (Lc[a + 2].x + Rc[a + 2].x), (Lc[a].y + Rc[a].y) + (Lc[a + 2].y + Rc[a + 2].y));
+                G[a] = mk<T>(fma(KW<T>::e(p, 1), Fx[a].x, KW<T>::e(p, 2) * Fy[a].x), fma(KW<T>::e(p, 1), Fx[a].y, KW<T>::e(p, 2) * Fy[a].y));
             }
         }
         // ---- psi(k) completes the z part of planes k-1 .. k-R -------------------------------------------
 #pragma unroll
         for (int e = 0; e < PR; ++e) {
-            AO[e].x = fma(KW<T>::w(p, R), v[e].x, AO[e].x);
-            AO[e].y = fma(KW<T>::w(p, R), v[e].y, AO[e].y);
+            AO[e].x = fma(KW<T>::w(p, 2, R), v[e].x, AO[e].x);
+            AO[e].y = fma(KW<T>::w(p, 2, R), v[e].y, AO[e].y);
             if (R == 2) {
-                AN[e].x = fma(KW<T>::w(p, 1), v[e].x, AN[e].x);
-                AN[e].y = fma(KW<T>::w(p, 1), v[e].y, AN[e].y);
+                AN[e].x = fma(KW<T>::w(p, 2, 1), v[e].x, AN[e].x);
+                AN[e].y = fma(KW<T>::w(p, 2, 1), v[e].y, AN[e].y);
             }
             if (HOC && MODE != MODE_PREP) {                     // the xz / yz edge neighbours of plane k-1 in plane k
-                AO[e].x = fma(KW<T>::w(p, 2), F[e].x, AO[e].x);
-                AO[e].y = fma(KW<T>::w(p, 2), F[e].y, AO[e].y);
+                AO[e].x += G[e].x;
+                AO[e].y += G[e].y;
             }
         }
         // ---- finish plane c = k - R: nonlinear term, stage combination (branch-free; stores predicated) ----
@@ -494,22 +501,22 @@ stage_kernel(const __grid_constant__ StageParams p) {
         for (int e = 0; e < PR; ++e) {
             C an;
             if (R == 2) {
-                an.x = KW<T>::w(p, 2) * PO[e].x;
-                an.y = KW<T>::w(p, 2) * PO[e].y;
-                an.x = fma(KW<T>::w(p, 1), PN[e].x, an.x);
-                an.y = fma(KW<T>::w(p, 1), PN[e].y, an.y);
+                an.x = KW<T>::w(p, 2, 2) * PO[e].x;
+                an.y = KW<T>::w(p, 2, 2) * PO[e].y;
+                an.x = fma(KW<T>::w(p, 2, 1), PN[e].x, an.x);
+                an.y = fma(KW<T>::w(p, 2, 1), PN[e].y, an.y);
             } else {
-                an.x = KW<T>::w(p, 1) * PO[e].x;
-                an.y = KW<T>::w(p, 1) * PO[e].y;
+                an.x = KW<T>::w(p, 2, 1) * PO[e].x;
+                an.y = KW<T>::w(p, 2, 1) * PO[e].y;
             }
-            AO[e].x = fma(KW<T>::w(p, 0), v[e].x, an.x);
-            AO[e].y = fma(KW<T>::w(p, 0), v[e].y, an.y);
+            AO[e].x = fma(KW<T>::c(p), v[e].x, an.x);
+            AO[e].y = fma(KW<T>::c(p), v[e].y, an.y);
             PO[e] = v[e];
             if (HOC && MODE != MODE_PREP) {
-                // faces of plane k, and the edges: diagonals of plane k + face sum of plane k-1
-                AO[e].x = fma(KW<T>::w(p, 1), F[e].x, fma(KW<T>::w(p, 2), E[e].x + FPV[e].x, AO[e].x));
-                AO[e].y = fma(KW<T>::w(p, 1), F[e].y, fma(KW<T>::w(p, 2), E[e].y + FPV[e].y, AO[e].y));
-                FPV[e] = F[e];
+                // faces and diagonals of plane k, and plane k-1's share of the xz / yz edges
+                AO[e].x = fma(KW<T>::w(p, 0, 1), Fx[e].x, fma(KW<T>::w(p, 1, 1), Fy[e].x, fma(KW<T>::e(p, 0), E[e].x, AO[e].x + GPV[e].x)));
+                AO[e].y = fma(KW<T>::w(p, 0, 1), Fx[e].y, fma(KW<T>::w(p, 1, 1), Fy[e].y, fma(KW<T>::e(p, 0), E[e].y, AO[e].y + GPV[e].y)));
+                GPV[e] = G[e];
             }
         }
         // ---- in-plane part (only planes of the stream itself are ever finished) ----------------------------------
@@ -522,8 +529,8 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 for (int a = 0; a < PR; ++a) {
                     const int d = r > a ? r - a : a - r;
                     if (d >= 1 && d <= R) {
-                        AO[a].x = fma(KW<T>::w(p, d), val.x, AO[a].x);
-                        AO[a].y = fma(KW<T>::w(p, d), val.y, AO[a].y);
+                        AO[a].x = fma(KW<T>::w(p, 0, d), val.x, AO[a].x);
+                        AO[a].y = fma(KW<T>::w(p, 0, d), val.y, AO[a].y);
                     }
                 }
             }
@@ -535,8 +542,8 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     if (cc == 0) continue;
                     const C val = lds_c(so + (unsigned)(a * (int)ROW_BYTES + cc * (int)ES), (C*)nullptr);
                     const int d = cc > 0 ? cc : -cc;
-                    AO[a].x = fma(KW<T>::w(p, d), val.x, AO[a].x);
-                    AO[a].y = fma(KW<T>::w(p, d), val.y, AO[a].y);
+                    AO[a].x = fma(KW<T>::w(p, 1, d), val.x, AO[a].x);
+                    AO[a].y = fma(KW<T>::w(p, 1, d), val.y, AO[a].y);
                 }
             }
         }

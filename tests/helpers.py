@@ -6,7 +6,7 @@ from oracle import gpe_oracle as O
 
 
 def oracle_objs(w, active=None):
-    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center)
+    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center, w.hy, w.hz)
     pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
     act = O.active_indices(box, pot, w.v_cut, w.mask_mode) if active is None else np.asarray(active, np.int64)
     return box, pot, act

@@ -316,3 +316,29 @@ def test_small_shell_1000_steps(P, dtype, stencil):
     else:
         ref = CO.COracle(box, pot, act, stencil).run_rk4(w.g, 0.0, w.dt, 1000, psi.astype(np.complex128))
     assert rel_max(sim.get_psi_host(), ref) < TOL_STEPS[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+@pytest.mark.parametrize("stencil", [7, 13, 19])
+def test_anisotropic_spacing(P, stencil, dtype):
+    """Anisotropic grids d_x != d_y != d_z (App. B, Eq. B1-B2): the mask, the operator with
+    per-axis weights (19-point: pair weights (d_i^2 + d_j^2)/12), RK4, the volume element of the reductions."""
+    tol = 1e-12 if dtype == "complex128" else 1e-5
+    w = I.small_shell(40, stencil, dtype).with_(hy=0.8 * 0.5, hz=1.3 * 0.5, delta0=14.0, delta1=20.0, t_ramp=0.02)
+    w = w.with_(h=0.5)
+    box, pot, act, grid, sim = _make(P, w)
+    assert act.size > 3000
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.random_psi(9, act.size).astype(sim.npdtype)
+    got = sim.apply_H(0.004, _dev(psi, dtype)).cpu().numpy()
+    assert rel_max(got, O.apply_H(og, pot, w.g, 0.004, psi.astype(np.complex128), stencil)) < tol
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    assert abs(sim.norm() - 1.0) < (1e-12 if dtype == "complex128" else 1e-6)     # h hy hz sum |psi|^2
+    sim.run_rk4(w.dt, 3)
+    ref = O.run_rk4(og, pot, w.g, 0.0, w.dt, 3, psi.astype(np.complex128), stencil)
+    assert rel_max(sim.get_psi_host(), ref) < tol
+    if dtype == "complex128":
+        e, eo = sim.energy(), O.energy(og, pot, w.g, sim.time, ref, stencil)
+        for k in eo:
+            assert abs(e[k] - eo[k]) <= 1e-11 * max(1.0, abs(eo[k])), k

@@ -41,7 +41,8 @@ def _compare_tables(w, active=None, zt=32):
 
 
 @pytest.mark.parametrize("wl", [I.config1(), I.small_shell(40, 13), I.small_shell(24, 7, aniso=False),
-                                I.small_shell(33, 13).with_(center=(0.3, -0.2, 0.1))])
+                                I.small_shell(33, 13).with_(center=(0.3, -0.2, 0.1)),
+                                I.small_shell(40, 13).with_(hy=0.4, hz=0.65)])
 def test_layout_tables_bit_exact(wl):
     _compare_tables(wl)
 

@@ -15,7 +15,7 @@ import gpe_inputs as I
 
 
 def _objs(w):
-    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center)
+    box = O.Box(w.nx, w.ny, w.nz, w.h, w.center, w.hy, w.hz)
     pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
     act = O.active_indices(box, pot, w.v_cut, w.mask_mode)
     return box, pot, act

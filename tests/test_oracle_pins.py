@@ -701,3 +701,54 @@ def test_P17_19pt_leading_error_is_isotropic():
         s = [-(4 / h ** 2) * math.sin(k * h / 2) ** 2 for k in kv]
         lam19 = sum(s) + h * h / 6 * (s[0] * s[1] + s[0] * s[2] + s[1] * s[2])
         assert abs(lam19 - (-9.0 + h * h * 81.0 / 12)) < 5e-5 * 9
+
+
+# ---- P18: anisotropic spacing d_x != d_y != d_z (App. B) -----------------------------------------
+def test_P18_anisotropic_spacing():
+    nx, ny, nz = 6, 7, 5
+    dx, dy, dz = 0.5, 0.8, 0.3
+    box = O.Box(nx, ny, nz, dx, (0.1, -0.2, 0.3), dy, dz)
+    full = np.arange(nx * ny * nz, dtype=np.int64)
+    grid = O.SparseGrid(box, full, 2)
+    # (a) 7-point: sine modes are exact eigenvectors, each axis with its own step (Eq. B1)
+    mode = (2, 3, 1)
+    psi = sine_mode(nx, ny, nz, mode).ravel()
+    lam = sum(-(4 / d ** 2) * math.sin(math.pi * m / (2 * (n + 1))) ** 2 for d, m, n in zip((dx, dy, dz), mode, (nx, ny, nz)))
+    assert np.max(np.abs(O.apply_T(grid, psi, 7) + 0.5 * lam * psi)) < 1e-12
+    # (b) Kronecker forms with per-axis second differences, rows / columns deleted, 7 / 13 / 19 points
+    eye = np.eye
+    k3 = lambda a, b, c: np.kron(np.kron(a, b), c)
+    for stencil in (7, 13, 19):
+        st = 7 if stencil == 19 else stencil
+        ddx, ddy, ddz = lap1d(nx, dx, st), lap1d(ny, dy, st), lap1d(nz, dz, st)
+        lap = k3(ddx, eye(ny), eye(nz)) + k3(eye(nx), ddy, eye(nz)) + k3(eye(nx), eye(ny), ddz)
+        if stencil == 19:
+            lap = lap + ((dx * dx + dy * dy) * k3(ddx, ddy, eye(nz)) + (dx * dx + dz * dz) * k3(ddx, eye(ny), ddz)
+                         + (dy * dy + dz * dz) * k3(eye(nx), ddy, ddz)) / 12
+        act = I.random_mask_lin(41, nx, ny, nz, 0.7)
+        g2 = O.SparseGrid(box, act, 2)
+        tmat = -0.5 * lap[np.ix_(act, act)]
+        phi = I.random_psi(42, act.size)
+        assert np.max(np.abs(O.apply_T(g2, phi, stencil) - tmat @ phi)) < 1e-12 * np.max(np.abs(tmat)) * 8
+        if stencil != 19:
+            mask = np.zeros(nx * ny * nz, bool)
+            mask[act] = True
+            dense = np.zeros(nx * ny * nz, np.complex128)
+            dense[act] = phi
+            got = O.dense_apply_T(box, mask.reshape(nx, ny, nz), dense.reshape(nx, ny, nz), stencil).ravel()[act]
+            assert np.max(np.abs(got - tmat @ phi)) < 1e-12 * np.max(np.abs(tmat)) * 8
+    # (c) coordinates, volume element, separable harmonic ground state
+    assert abs(O.norm(grid, np.ones(full.size, np.complex128)) - full.size * dx * dy * dz) < 1e-12
+    v = O.potential_at(box, O.Potential(kind=O.HARMONIC, ax=1.0, ay=2.0, az=3.0), full, 0.0).reshape(nx, ny, nz)
+    x = (np.arange(nx) - 0.5 * (nx - 1)) * dx + 0.1
+    y = (np.arange(ny) - 0.5 * (ny - 1)) * dy - 0.2
+    z = (np.arange(nz) - 0.5 * (nz - 1)) * dz + 0.3
+    assert np.max(np.abs(v - 0.5 * (x[:, None, None] ** 2 + 2 * y[None, :, None] ** 2 + 3 * z[None, None, :] ** 2))) < 1e-14
+    n = 16
+    boxh = O.Box(n, n, n, 0.5, (0.0, 0.0, 0.0), 0.6, 0.7)
+    gh = O.SparseGrid(boxh, np.arange(n ** 3, dtype=np.int64), 1)
+    es, vs = zip(*[ho_ground_state_1d(n, d, 7) for d in (0.5, 0.6, 0.7)])
+    psi = (vs[0][:, None, None] * vs[1][None, :, None] * vs[2][None, None, :]).ravel().astype(np.complex128)
+    psi /= math.sqrt(O.norm(gh, psi))
+    e = O.energy(gh, O.Potential(kind=O.HARMONIC), 0.0, 0.0, psi, 7)
+    assert abs(e["total"] - sum(es)) < 1e-12 and abs(e["mu"] - sum(es)) < 1e-12

@@ -52,6 +52,10 @@ extern "C" {
 
 #define GPE_C64 0  /* complex64 state; coordinates, V and all reductions still fp64           */
 #define GPE_C128 1 /* complex128 state                                                        */
+#define GPE_R64 2  /* real float64 state for ground states (imaginary time "does not require the
+                      wavefunction to be complex"): half the bytes of complex128; the operator, the imaginary-time
+                      calls, the reductions and re-gridding only -- the Runge-Kutta calls return UNSUPPORTED.
+                      Canonical arrays hold n_active doubles. */
 
 typedef struct gpe_grid gpe_grid; /* opaque: active set + layout tables (host, and device once a sim exists) */
 typedef struct gpe_sim gpe_sim;   /* opaque: one wavefunction evolving on a grid                              */
@@ -226,7 +230,7 @@ int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream);
  * Three stage launches per iteration (pointwise Eq. 7 with the lazily applied scale of the previous iteration;
  * Euler half step; Euler half step + Eq. 7 + block partial sums) and a one-block finalise; exp(-V dt/2) is
  * evaluated analytically per point (no propagator array is read).  The scale is flushed at the end of the call.
- * psi stays complex (the real-valued variant of :67 is not built).  Same arguments and errors as gpe_run_imag. */
+ * With a GPE_R64 sim the state is real (:67).  Same arguments and errors as gpe_run_imag. */
 int gpe_imag_split_step(gpe_sim* s, double dt, void* stream);
 int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 

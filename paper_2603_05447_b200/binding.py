@@ -16,7 +16,7 @@ from . import build as _build
 
 HARMONIC, DRESSED = 0, 1
 MASK_AT_DELTA0, MASK_AT_DELTA1, MASK_UNION = 0, 1, 2
-C64, C128 = 0, 1
+C64, C128, R64 = 0, 1, 2
 
 ERR_NAMES = {-1: "GPE_ERR_INVALID_ARG", -2: "GPE_ERR_OUT_OF_MEMORY", -3: "GPE_ERR_CUDA",
              -4: "GPE_ERR_UNSUPPORTED", -5: "GPE_ERR_STATE"}
@@ -186,9 +186,12 @@ class Sim:
         self.grid = grid
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self.dtype_code = C128 if str(dtype) in ("complex128", "torch.complex128") else C64
-        self.cdtype = torch.complex128 if self.dtype_code == C128 else torch.complex64
-        self.npdtype = np.complex128 if self.dtype_code == C128 else np.complex64
+        name = str(dtype).replace("torch.", "")
+        if name not in ("complex128", "complex64", "float64"):
+            raise ValueError(f"dtype must be complex128, complex64 or float64 (real-valued ground states), not {dtype}")
+        self.dtype_code = {"complex128": C128, "complex64": C64, "float64": R64}[name]
+        self.cdtype = {C128: torch.complex128, C64: torch.complex64, R64: torch.float64}[self.dtype_code]
+        self.npdtype = {C128: np.complex128, C64: np.complex64, R64: np.float64}[self.dtype_code]
         self.n = grid.n_active
         nbytes = C.c_size_t()
         _check(lib().gpe_sim_state_bytes(grid._h, C.c_int(self.dtype_code), C.byref(nbytes)))

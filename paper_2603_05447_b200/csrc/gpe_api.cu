@@ -76,6 +76,12 @@ double cell_volume(const gpe_box& b) { return b.h * (b.hy > 0.0 ? b.hy : b.h) * 
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// GPE_R64: 8-byte elements.  Copies move them with the 8-byte (complex64) kernels; sums of squares and the scaling
+// treat the array as ceil(n/2) complex128 values (buffers are zero-filled and 256-byte padded, the odd tail is 0).
+int copy_dtype(int dtype) { return dtype == GPE_R64 ? GPE_C64 : dtype; }
+int pair_dtype(int dtype) { return dtype == GPE_R64 ? GPE_C128 : dtype; }
+int64_t pair_count(int dtype, int64_t n) { return dtype == GPE_R64 ? (n + 1) / 2 : n; }
+
 size_t buf_bytes(int64_t n, int dtype) { return align_up((size_t)(n > 0 ? n : 1) * (dtype == GPE_C128 ? 16 : 8), 256); }
 
 PotDev pot_dev(const gpe_sim* s, double t) {
@@ -413,7 +419,7 @@ int gpe_grid_layout_tables(const gpe_grid* g, const gpe_layout_tables* o) {
 
 int gpe_sim_state_bytes(const gpe_grid* g, int dtype, size_t* out) {
     if (!g || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
-    if (dtype != GPE_C64 && dtype != GPE_C128) return fail(GPE_ERR_INVALID_ARG, "unknown dtype");
+    if (dtype != GPE_C64 && dtype != GPE_C128 && dtype != GPE_R64) return fail(GPE_ERR_INVALID_ARG, "unknown dtype");
     *out = 5 * buf_bytes(g->h.n_active, dtype);
     return GPE_OK;
 }
@@ -421,7 +427,7 @@ int gpe_sim_state_bytes(const gpe_grid* g, int dtype, size_t* out) {
 int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_target, void* dev_state,
                    size_t state_bytes, void* stream, gpe_sim** out) {
     if (!g || !dev_state || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
-    if (dtype != GPE_C64 && dtype != GPE_C128) return fail(GPE_ERR_INVALID_ARG, "unknown dtype");
+    if (dtype != GPE_C64 && dtype != GPE_C128 && dtype != GPE_R64) return fail(GPE_ERR_INVALID_ARG, "unknown dtype");
     if (stencil != 7 && stencil != 13 && stencil != 19) return fail(GPE_ERR_INVALID_ARG, "stencil must be 7, 13 or 19");
     if (!(n_target > 0.0)) return fail(GPE_ERR_INVALID_ARG, "n_target must be > 0");
     const int radius = stencil == 13 ? 2 : 1;
@@ -480,14 +486,14 @@ int gpe_sim_destroy(gpe_sim* s) {
 
 int gpe_set_psi(gpe_sim* s, const void* dev_psi_canonical, void* stream) {
     if (!s || (!dev_psi_canonical && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
-    KL(launch_pack(s->dtype, dev_psi_canonical, s->buf[0], s->grid->d_perm, s->n, stream));
+    KL(launch_pack(copy_dtype(s->dtype), dev_psi_canonical, s->buf[0], s->grid->d_perm, s->n, stream));
     if (s->n > 0) s->launches += 1;
     return GPE_OK;
 }
 
 int gpe_get_psi(gpe_sim* s, void* dev_psi_canonical, void* stream) {
     if (!s || (!dev_psi_canonical && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
-    KL(launch_unpack(s->dtype, s->buf[0], dev_psi_canonical, s->grid->d_perm, s->n, stream));
+    KL(launch_unpack(copy_dtype(s->dtype), s->buf[0], dev_psi_canonical, s->grid->d_perm, s->n, stream));
     if (s->n > 0) s->launches += 1;
     return GPE_OK;
 }
@@ -516,9 +522,9 @@ int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     e = cudaMemcpyAsync(d_map, map.data(), map.size() * sizeof(int64_t), cudaMemcpyHostToDevice, st);
     int rc = 0;
-    if (e == cudaSuccess && src->n > 0) rc = launch_unpack(src->dtype, src->buf[0], src->staging, src->grid->d_perm, src->n, stream);
-    if (e == cudaSuccess && !rc) rc = launch_remap(dst->dtype, src->staging, dst->staging, d_map, dst->n, stream);
-    if (e == cudaSuccess && !rc) rc = launch_pack(dst->dtype, dst->staging, dst->buf[0], dst->grid->d_perm, dst->n, stream);
+    if (e == cudaSuccess && src->n > 0) rc = launch_unpack(copy_dtype(src->dtype), src->buf[0], src->staging, src->grid->d_perm, src->n, stream);
+    if (e == cudaSuccess && !rc) rc = launch_remap(copy_dtype(dst->dtype), src->staging, dst->staging, d_map, dst->n, stream);
+    if (e == cudaSuccess && !rc) rc = launch_pack(copy_dtype(dst->dtype), dst->staging, dst->buf[0], dst->grid->d_perm, dst->n, stream);
     if (e == cudaSuccess && !rc) e = cudaStreamSynchronize(st);   // the table is freed below
     cudaFree(d_map);
     if (e != cudaSuccess) return cuda_fail(e, "gpe_remap_psi");
@@ -569,17 +575,18 @@ int gpe_apply_H(gpe_sim* s, double t, const void* dev_in_canonical, void* dev_ou
     const size_t bytes = (size_t)s->n * s->csize;
     if (a < b + bytes && b < a + bytes) return fail(GPE_ERR_INVALID_ARG, "in and out overlap");
     // scratch: C holds the packed input, D the packed result; the sim's psi (A) is untouched
-    KL(launch_pack(s->dtype, dev_in_canonical, s->buf[2], s->grid->d_perm, s->n, stream));
+    KL(launch_pack(copy_dtype(s->dtype), dev_in_canonical, s->buf[2], s->grid->d_perm, s->n, stream));
     s->launches += 1;
     int rc = stage(s, MODE_APPLY, t, 0.0, s->buf[2], nullptr, s->buf[3], nullptr, stream);
     if (rc) return rc;
-    KL(launch_unpack(s->dtype, s->buf[3], dev_out_canonical, s->grid->d_perm, s->n, stream));
+    KL(launch_unpack(copy_dtype(s->dtype), s->buf[3], dev_out_canonical, s->grid->d_perm, s->n, stream));
     s->launches += 1;
     return GPE_OK;
 }
 
 int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (s->dtype == GPE_R64) return fail(GPE_ERR_UNSUPPORTED, "real-time evolution needs a complex state (GPE_C64 / GPE_C128)");
     if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
     const double t0 = s->t;
     for (int64_t n = 0; n < nsteps; ++n) {
@@ -594,6 +601,7 @@ int gpe_step_rk4(gpe_sim* s, double dt, void* stream) { return gpe_run_rk4(s, dt
 
 int gpe_run_rkhe3(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (s->dtype == GPE_R64) return fail(GPE_ERR_UNSUPPORTED, "real-time evolution needs a complex state (GPE_C64 / GPE_C128)");
     if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
     const double t0 = s->t;
     for (int64_t n = 0; n < nsteps; ++n) {
@@ -608,6 +616,7 @@ int gpe_step_rkhe3(gpe_sim* s, double dt, void* stream) { return gpe_run_rkhe3(s
 
 int gpe_run_rkck(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (s->dtype == GPE_R64) return fail(GPE_ERR_UNSUPPORTED, "real-time evolution needs a complex state (GPE_C64 / GPE_C128)");
     if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
     if (s->n > 0 && nsteps > 0) {
         for (int k = 0; k < 2; ++k) {
@@ -642,7 +651,7 @@ int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
         std::swap(s->buf[0], s->buf[1]);
     }
     // flush the lazy scale so that every other call sees a normalised state
-    KL(launch_scale(s->dtype, s->buf[0], s->n, s->d_sums + NACC, stream));
+    KL(launch_scale(pair_dtype(s->dtype), s->buf[0], pair_count(s->dtype, s->n), s->d_sums + NACC, stream));
     KL(launch_set_scalar(s->d_sums + NACC, 1.0, stream));
     s->launches += 2;
     return GPE_OK;
@@ -666,7 +675,7 @@ int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
         s->launches += 1;
         std::swap(s->buf[0], s->buf[1]);
     }
-    KL(launch_scale(s->dtype, s->buf[0], s->n, s->d_sums + NACC, stream));
+    KL(launch_scale(pair_dtype(s->dtype), s->buf[0], pair_count(s->dtype, s->n), s->d_sums + NACC, stream));
     KL(launch_set_scalar(s->d_sums + NACC, 1.0, stream));
     s->launches += 2;
     return GPE_OK;
@@ -678,8 +687,8 @@ int gpe_norm(gpe_sim* s, double* out_host, void* stream) {
     if (!s || !out_host) return fail(GPE_ERR_INVALID_ARG, "null argument");
     const double h3 = cell_volume(s->grid->h.box);
     if (s->n == 0) { *out_host = 0.0; return GPE_OK; }
-    KL(launch_norm_partials(s->dtype, s->buf[0], s->n, s->d_partials, stream));
-    KL(launch_finalize(s->d_partials, norm_blocks(s->n), s->d_sums, nullptr, s->n_target, h3, stream));
+    KL(launch_norm_partials(pair_dtype(s->dtype), s->buf[0], pair_count(s->dtype, s->n), s->d_partials, stream));
+    KL(launch_finalize(s->d_partials, norm_blocks(pair_count(s->dtype, s->n)), s->d_sums, nullptr, s->n_target, h3, stream));
     s->launches += 2;
     double sums[NACC];
     int rc = sums_to_host(s, sums, stream);

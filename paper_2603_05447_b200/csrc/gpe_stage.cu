@@ -42,12 +42,26 @@ template <typename T> __device__ __forceinline__ typename CxOf<T>::type mk(T a, 
 template <> __device__ __forceinline__ double2 mk<double>(double a, double b) { return make_double2(a, b); }
 template <> __device__ __forceinline__ float2 mk<float>(float a, float b) { return make_float2(a, b); }
 
+// Storage element of a REAL-valued state (ground states by imaginary time need no imaginary part):
+// 8 bytes in memory and in shared memory, widened to (x, 0) in registers, so every kernel below runs unchanged
+// on half the bytes.
+struct Re8 { double x; };
+template <typename T, bool REAL> struct ElemOf { using type = typename CxOf<T>::type; };
+template <> struct ElemOf<double, true> { using type = Re8; };
+__device__ __forceinline__ double2 to_elem(double2 v, double2*) { return v; }
+__device__ __forceinline__ float2 to_elem(float2 v, float2*) { return v; }
+__device__ __forceinline__ Re8 to_elem(double2 v, Re8*) { Re8 r; r.x = v.x; return r; }
+
 // cp.async of one complex value with zero fill (src-size 0 reads nothing and writes zeros: Dirichlet psi = 0)
 __device__ __forceinline__ void cp_async_zfill(unsigned smem_dst, const double2* src, bool valid) {
     const int sz = valid ? 16 : 0;
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_dst), "l"(src), "r"(sz) : "memory");
 }
 __device__ __forceinline__ void cp_async_zfill(unsigned smem_dst, const float2* src, bool valid) {
+    const int sz = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_dst), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_zfill(unsigned smem_dst, const Re8* src, bool valid) {
     const int sz = valid ? 8 : 0;
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_dst), "l"(src), "r"(sz) : "memory");
 }
@@ -63,6 +77,12 @@ __device__ __forceinline__ double2 lds_c(unsigned addr, double2*) {
 __device__ __forceinline__ float2 lds_c(unsigned addr, float2*) {
     float2 v;
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double2 lds_c(unsigned addr, Re8*) {
+    double2 v;
+    asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v.x) : "r"(addr));
+    v.y = 0.0;
     return v;
 }
 __device__ __forceinline__ uint2 lds_u2(unsigned addr) {
@@ -109,12 +129,12 @@ constexpr int STAGE_WARPS = STAGE_THREADS / 32;
 
 // Shared memory of one stream.  Plane slot: (8+2R) rows (x) of PY values, the tile at rows/cols R..R+7 and
 // the star halo around it.
-template <typename T, int R, bool AUX, bool HOC = false> struct Geo {
+template <typename T, int R, bool AUX, bool HOC = false, bool REAL = false> struct Geo {
     static constexpr int NT = HOC ? NTILE : 5;               // tiles whose slab tables are staged
-    static constexpr int ES = 2 * (int)sizeof(T);
+    static constexpr int ES = (REAL ? 1 : 2) * (int)sizeof(T);
     static constexpr int ROWS = 8 + 2 * R;
     // row pitch in values; 8-byte values are read by half-warps (two rows, 2 apart): 2 PY 8 = 64 (mod 128) bytes
-    static constexpr int PY = sizeof(T) == 4 ? 12 : 8 + 2 * R;
+    static constexpr int PY = ES == 8 ? 12 : 8 + 2 * R;
     static constexpr int PLANE = ROWS * PY;                 // values per slot
     static constexpr int NE = KZMAX + 2 * R;                // table entries per tile
     static constexpr int NSLOT = pf_of(R) + 1;              // ring of plane slots per stream
@@ -141,13 +161,15 @@ template <> struct KW<float> {
 
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
 
-template <typename T, int R, int MODE, int PR, bool HOC>
+template <typename T, int R, int MODE, int PR, bool HOC, bool REAL>
 __global__ void __launch_bounds__(STAGE_THREADS, 16)
 stage_kernel(const __grid_constant__ StageParams p) {
     static_assert(!HOC || (R == 1 && PR == 2), "the 19-point stencil has radius 1 and runs with a warp per stream");
-    using C = typename CxOf<T>::type;
+    static_assert(!REAL || sizeof(T) == 8, "the real-valued state is fp64");
+    using C = typename CxOf<T>::type;                      // value in registers
+    using EL = typename ElemOf<T, REAL>::type;             // value in memory
     constexpr bool HAS_AUX = mode_has_aux(MODE);
-    using G = Geo<T, R, HAS_AUX, HOC>;
+    using G = Geo<T, R, HAS_AUX, HOC, REAL>;
     constexpr int NT = G::NT;
     constexpr int PF = pf_of(R), NSLOT = G::NSLOT, NAUX = G::NAUX;
     constexpr unsigned ES = G::ES;
@@ -237,8 +259,8 @@ stage_kernel(const __grid_constant__ StageParams p) {
     // of the diagonal tile, bit cbit of its high (t < 2) or low mask word
     const int cbit = t == 0 ? 31 : (t == 1 ? 24 : (t == 2 ? 7 : 0));
     const unsigned coff = (unsigned)G::at((t & 2) ? 8 : -1, (t & 1) ? 8 : -1) * ES;
-    const C* __restrict__ in = reinterpret_cast<const C*>(p.in);
-    const C* __restrict__ auxp = reinterpret_cast<const C*>(p.aux);
+    const EL* __restrict__ in = reinterpret_cast<const EL*>(p.in);
+    const EL* __restrict__ auxp = reinterpret_cast<const EL*>(p.aux);
 
     // potential: u = qxy[e] + qz(plane); qxy = 1/2 (ax x^2 + ay y^2) of the patch points
     double qxy[PR];
@@ -354,7 +376,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
         if (MODE == MODE_LC) {
 #pragma unroll
             for (int e = 0; e < PR; ++e) lcs[e] = mk<T>((T)0, (T)0);
-            if (cany) {
+            if (cany && !REAL) {
 #pragma unroll
                 for (int j = 0; j < MAX_LC_AUX; ++j) {
                     if (j < p.n_aux) {
@@ -363,7 +385,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
 #pragma unroll
                         for (int e = 0; e < PR; ++e) {
                             if ((cword >> (rb0 + 8 * e)) & 1u) {
-                                const C a = __ldg(aj + (cbase + (unsigned)__popc(cword & bm[e])));
+                                const C a = __ldg(aj + (REAL ? 0u : cbase + (unsigned)__popc(cword & bm[e])));
                                 lcs[e].x = fma(cj, a.x, lcs[e].x);
                                 lcs[e].y = fma(cj, a.y, lcs[e].y);
                             }
@@ -375,7 +397,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
         // ---- psi(k) of the patch ------------------------------------------------------------------------
         C v[PR];
 #pragma unroll
-        for (int e = 0; e < PR; ++e) v[e] = lds_c(so + (unsigned)e * ROW_BYTES, (C*)nullptr);
+        for (int e = 0; e < PR; ++e) v[e] = lds_c(so + (unsigned)e * ROW_BYTES, (EL*)nullptr);
         // ---- V(r,t) of plane c: depends on coordinates only, so its dependency chains (one per patch point,
         //      interleaved) are issued here and overlap the shared-memory latency of psi(k) --------------------
         double vpot[PR];
@@ -396,9 +418,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
             C Lc[4], Rc[4], Mc[4];                              // columns ly-1, ly+1, ly of rows -1 .. 2 of the patch
 #pragma unroll
             for (int r = -1; r <= 2; ++r) {
-                Lc[r + 1] = lds_c(so + (unsigned)(r * (int)ROW_BYTES - (int)ES), (C*)nullptr);
-                Rc[r + 1] = lds_c(so + (unsigned)(r * (int)ROW_BYTES + (int)ES), (C*)nullptr);
-                Mc[r + 1] = (r == 0 || r == 1) ? v[r == 1 ? 1 : 0] : lds_c(so + (unsigned)(r * (int)ROW_BYTES), (C*)nullptr);
+                Lc[r + 1] = lds_c(so + (unsigned)(r * (int)ROW_BYTES - (int)ES), (EL*)nullptr);
+                Rc[r + 1] = lds_c(so + (unsigned)(r * (int)ROW_BYTES + (int)ES), (EL*)nullptr);
+                Mc[r + 1] = (r == 0 || r == 1) ? v[r == 1 ? 1 : 0] : lds_c(so + (unsigned)(r * (int)ROW_BYTES), (EL*)nullptr);
             }
 #pragma unroll
             for (int a = 0; a < PR; ++a) {
@@ -428,7 +450,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
 #pragma unroll
             for (int e = 0; e < PR; ++e) {
                 av[e] = mk<T>((T)0, (T)0);
-                if (HAS_AUX) av[e] = lds_c(auxring + al * (64u * ES) + aux_off + (unsigned)e * (8u * ES), (C*)nullptr);
+                if (HAS_AUX) av[e] = lds_c(auxring + al * (64u * ES) + aux_off + (unsigned)e * (8u * ES), (EL*)nullptr);
             }
 #pragma unroll
             for (int e = 0; e < PR; ++e) {
@@ -461,7 +483,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
                         const double o2 = (double)o.x * (double)o.x + (double)o.y * (double)o.y;
                         acc[0] += on ? o2 : 0.0;
                     }
-                    if (on) reinterpret_cast<C*>(p.out1)[pos] = o;
+                    if (on) reinterpret_cast<EL*>(p.out1)[pos] = to_elem(o, (EL*)nullptr);
                     continue;
                 }
                 const T diag = (T)fma(gsc, (double)a2, vpot[e]);
@@ -490,10 +512,10 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     if (MODE == MODE_S2) {
                         const T b0 = (T)p.comb[0], b1 = (T)p.comb[1], b2 = (T)p.comb[2];
                         const C o2 = mk<T>(fma(b2, o.x, fma(b1, cv.x, b0 * av[e].x)), fma(b2, o.y, fma(b1, cv.y, b0 * av[e].y)));
-                        if (on) reinterpret_cast<C*>(p.out2)[pos] = o2;
+                        if (on) reinterpret_cast<EL*>(p.out2)[pos] = to_elem(o2, (EL*)nullptr);
                     }
                 }
-                if (on) reinterpret_cast<C*>(p.out1)[pos] = o;
+                if (on) reinterpret_cast<EL*>(p.out1)[pos] = to_elem(o, (EL*)nullptr);
             }
         }
         // ---- the oldest set becomes the set of plane k: z-backward part, centre ---------------------------------
@@ -524,7 +546,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
             // x direction: source rows r = -R .. PR-1+R of column ly; rows 0..PR-1 are the patch itself
 #pragma unroll
             for (int r = -R; r <= PR - 1 + R; ++r) {
-                const C val = (r >= 0 && r < PR) ? v[r < 0 ? 0 : (r < PR ? r : 0)] : lds_c(so + (unsigned)(r * (int)ROW_BYTES), (C*)nullptr);
+                const C val = (r >= 0 && r < PR) ? v[r < 0 ? 0 : (r < PR ? r : 0)] : lds_c(so + (unsigned)(r * (int)ROW_BYTES), (EL*)nullptr);
 #pragma unroll
                 for (int a = 0; a < PR; ++a) {
                     const int d = r > a ? r - a : a - r;
@@ -540,7 +562,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
 #pragma unroll
                 for (int cc = -R; cc <= R; ++cc) {
                     if (cc == 0) continue;
-                    const C val = lds_c(so + (unsigned)(a * (int)ROW_BYTES + cc * (int)ES), (C*)nullptr);
+                    const C val = lds_c(so + (unsigned)(a * (int)ROW_BYTES + cc * (int)ES), (EL*)nullptr);
                     const int d = cc > 0 ? cc : -cc;
                     AO[a].x = fma(KW<T>::w(p, 1, d), val.x, AO[a].x);
                     AO[a].y = fma(KW<T>::w(p, 1, d), val.y, AO[a].y);
@@ -586,55 +608,80 @@ stage_kernel(const __grid_constant__ StageParams p) {
 // 9.8e10 stage updates/s on cfg 4 against 1.2e11 with 2 rows (twice the shared memory per warp: 11 warps per SM)
 template <typename T> constexpr int rows_per_lane() { return 2; }
 
-template <typename T, int R, int MODE, bool HOC> constexpr size_t stage_smem() {
-    return (size_t)(STAGE_WARPS * rows_per_lane<T>() / 2) * Geo<T, R, mode_has_aux(MODE), HOC>::STREAM_BYTES;
+template <typename T, int R, int MODE, bool HOC, bool REAL> constexpr size_t stage_smem() {
+    return (size_t)(STAGE_WARPS * rows_per_lane<T>() / 2) * Geo<T, R, mode_has_aux(MODE), HOC, REAL>::STREAM_BYTES;
 }
 
-template <typename T, int R, int MODE, bool HOC>
+template <typename T, int R, int MODE, bool HOC, bool REAL>
 cudaError_t launch_one(const StageParams& p, cudaStream_t st) {
     constexpr int spb = STAGE_WARPS * rows_per_lane<T>() / 2;   // streams per block
     const int nblk = (p.n_work + spb - 1) / spb;
-    stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC><<<nblk, STAGE_THREADS, stage_smem<T, R, MODE, HOC>(), st>>>(p);
+    stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC, REAL><<<nblk, STAGE_THREADS, stage_smem<T, R, MODE, HOC, REAL>(), st>>>(p);
     return cudaGetLastError();
 }
 
 template <typename T, int R, bool HOC>
 cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
     switch (mode) {
-        case MODE_APPLY: return launch_one<T, R, MODE_APPLY, HOC>(p, st);
-        case MODE_S1: return launch_one<T, R, MODE_S1, HOC>(p, st);
-        case MODE_S2: return launch_one<T, R, MODE_S2, HOC>(p, st);
-        case MODE_S3: return launch_one<T, R, MODE_S3, HOC>(p, st);
-        case MODE_S4: return launch_one<T, R, MODE_S4, HOC>(p, st);
-        case MODE_IMAG: return launch_one<T, R, MODE_IMAG, HOC>(p, st);
-        case MODE_ENERGY: return launch_one<T, R, MODE_ENERGY, HOC>(p, st);
-        case MODE_PREP: return launch_one<T, R, MODE_PREP, HOC>(p, st);
-        case MODE_KIN: return launch_one<T, R, MODE_KIN, HOC>(p, st);
-        case MODE_SPLITB: return launch_one<T, R, MODE_SPLITB, HOC>(p, st);
-        case MODE_LC: return launch_one<T, R, MODE_LC, HOC>(p, st);
+        case MODE_APPLY: return launch_one<T, R, MODE_APPLY, HOC, false>(p, st);
+        case MODE_S1: return launch_one<T, R, MODE_S1, HOC, false>(p, st);
+        case MODE_S2: return launch_one<T, R, MODE_S2, HOC, false>(p, st);
+        case MODE_S3: return launch_one<T, R, MODE_S3, HOC, false>(p, st);
+        case MODE_S4: return launch_one<T, R, MODE_S4, HOC, false>(p, st);
+        case MODE_IMAG: return launch_one<T, R, MODE_IMAG, HOC, false>(p, st);
+        case MODE_ENERGY: return launch_one<T, R, MODE_ENERGY, HOC, false>(p, st);
+        case MODE_PREP: return launch_one<T, R, MODE_PREP, HOC, false>(p, st);
+        case MODE_KIN: return launch_one<T, R, MODE_KIN, HOC, false>(p, st);
+        case MODE_SPLITB: return launch_one<T, R, MODE_SPLITB, HOC, false>(p, st);
+        case MODE_LC: return launch_one<T, R, MODE_LC, HOC, false>(p, st);
     }
     return cudaErrorInvalidValue;
 }
 
-template <typename T, int R, int MODE, bool HOC>
+// real-valued fp64 state: the operator and the imaginary-time modes only (real time needs the imaginary part)
+template <int R, bool HOC>
+cudaError_t launch_mode_real(int mode, const StageParams& p, cudaStream_t st) {
+    switch (mode) {
+        case MODE_APPLY: return launch_one<double, R, MODE_APPLY, HOC, true>(p, st);
+        case MODE_IMAG: return launch_one<double, R, MODE_IMAG, HOC, true>(p, st);
+        case MODE_ENERGY: return launch_one<double, R, MODE_ENERGY, HOC, true>(p, st);
+        case MODE_PREP: return launch_one<double, R, MODE_PREP, HOC, true>(p, st);
+        case MODE_KIN: return launch_one<double, R, MODE_KIN, HOC, true>(p, st);
+        case MODE_SPLITB: return launch_one<double, R, MODE_SPLITB, HOC, true>(p, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <typename T, int R, int MODE, bool HOC, bool REAL>
 cudaError_t set_attr() {
-    return cudaFuncSetAttribute(stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)stage_smem<T, R, MODE, HOC>());
+    return cudaFuncSetAttribute(stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC, REAL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)stage_smem<T, R, MODE, HOC, REAL>());
 }
 template <typename T, int R, bool HOC>
 cudaError_t set_attr_modes() {
     cudaError_t e;
-    if ((e = set_attr<T, R, MODE_APPLY, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_S1, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_S2, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_S3, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_S4, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_IMAG, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_ENERGY, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_PREP, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_KIN, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_SPLITB, HOC>())) return e;
-    if ((e = set_attr<T, R, MODE_LC, HOC>())) return e;
+    if ((e = set_attr<T, R, MODE_APPLY, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_S1, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_S2, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_S3, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_S4, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_IMAG, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_ENERGY, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_PREP, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_KIN, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_SPLITB, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_LC, HOC, false>())) return e;
+    return cudaSuccess;
+}
+template <int R, bool HOC>
+cudaError_t set_attr_modes_real() {
+    cudaError_t e;
+    if ((e = set_attr<double, R, MODE_APPLY, HOC, true>())) return e;
+    if ((e = set_attr<double, R, MODE_IMAG, HOC, true>())) return e;
+    if ((e = set_attr<double, R, MODE_ENERGY, HOC, true>())) return e;
+    if ((e = set_attr<double, R, MODE_PREP, HOC, true>())) return e;
+    if ((e = set_attr<double, R, MODE_KIN, HOC, true>())) return e;
+    if ((e = set_attr<double, R, MODE_SPLITB, HOC, true>())) return e;
     return cudaSuccess;
 }
 
@@ -645,10 +692,10 @@ int stage_max_planes() { return KZMAX; }
 // variant: 1 = 7-point, 2 = 13-point, 3 = 19-point (gpe_internal.h)
 size_t stage_smem_bytes(int dtype, int variant) {   // largest over the modes (the aux-carrying RK stages)
     if (dtype == GPE_C128)
-        return variant == 1 ? stage_smem<double, 1, MODE_S2, false>()
-                            : (variant == 2 ? stage_smem<double, 2, MODE_S2, false>() : stage_smem<double, 1, MODE_S2, true>());
-    return variant == 1 ? stage_smem<float, 1, MODE_S2, false>()
-                        : (variant == 2 ? stage_smem<float, 2, MODE_S2, false>() : stage_smem<float, 1, MODE_S2, true>());
+        return variant == 1 ? stage_smem<double, 1, MODE_S2, false, false>()
+                            : (variant == 2 ? stage_smem<double, 2, MODE_S2, false, false>() : stage_smem<double, 1, MODE_S2, true, false>());
+    return variant == 1 ? stage_smem<float, 1, MODE_S2, false, false>()
+                        : (variant == 2 ? stage_smem<float, 2, MODE_S2, false, false>() : stage_smem<float, 1, MODE_S2, true, false>());
 }
 
 int kernels_configure() {
@@ -659,6 +706,9 @@ int kernels_configure() {
     if ((e = set_attr_modes<float, 1, false>())) return (int)e;
     if ((e = set_attr_modes<float, 2, false>())) return (int)e;
     if ((e = set_attr_modes<float, 1, true>())) return (int)e;
+    if ((e = set_attr_modes_real<1, false>())) return (int)e;
+    if ((e = set_attr_modes_real<2, false>())) return (int)e;
+    if ((e = set_attr_modes_real<1, true>())) return (int)e;
     return 0;
 }
 
@@ -673,6 +723,12 @@ cudaError_t launch_variant(int variant, int mode, const StageParams& p, cudaStre
 int launch_stage(int dtype, int variant, int mode, const StageParams& p, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     if (p.n_work <= 0) return 0;
+    if (dtype == GPE_R64) {
+        if (variant == 1) return (int)launch_mode_real<1, false>(mode, p, st);
+        if (variant == 2) return (int)launch_mode_real<2, false>(mode, p, st);
+        if (variant == 3) return (int)launch_mode_real<1, true>(mode, p, st);
+        return (int)cudaErrorInvalidValue;
+    }
     return (int)(dtype == GPE_C128 ? launch_variant<double>(variant, mode, p, st) : launch_variant<float>(variant, mode, p, st));
 }
 

@@ -342,3 +342,47 @@ def test_anisotropic_spacing(P, stencil, dtype):
         e, eo = sim.energy(), O.energy(og, pot, w.g, sim.time, ref, stencil)
         for k in eo:
             assert abs(e[k] - eo[k]) <= 1e-11 * max(1.0, abs(eo[k])), k
+
+
+@pytest.mark.parametrize("stencil", [7, 13, 19])
+def test_real_valued_ground_state_mode(P, stencil):
+    """Real float64 state (imaginary time "does not require the wavefunction to be complex"): the
+    operator, both imaginary-time schemes, norm, energy and re-gridding on half the bytes; the oracle runs the
+    same real initial state as complex128 and must stay real exactly."""
+    w = I.small_shell(40, stencil)
+    box, pot, act, grid, _ = _make(P, w)
+    sim = P.Sim(grid, "float64", stencil, w.g)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = np.abs(I.make_psi0(w, act)) * (1.0 + 0.1 * np.cos(np.arange(act.size)))
+    psi = psi / np.sqrt(O.norm(og, psi.astype(np.complex128)))
+    import torch
+    got = sim.apply_H(0.0, torch.from_numpy(psi).to("cuda:0")).cpu().numpy()
+    ref = O.apply_H(og, pot, w.g, 0.0, psi.astype(np.complex128), stencil)
+    assert np.all(ref.imag == 0) and rel_max(got, ref.real) < 1e-12
+    sim.set_psi_host(psi)
+    assert np.array_equal(sim.get_psi_host(), psi)
+    assert abs(sim.norm() - 1.0) < 1e-13
+    sim.run_imag(1e-3, 7)
+    ref = O.run_imag(og, pot, w.g, 0.0, 1e-3, 7, psi.astype(np.complex128), stencil)
+    assert np.all(ref.imag == 0) and rel_max(sim.get_psi_host(), ref.real) < 1e-12
+    e, eo = sim.energy(), O.energy(og, pot, w.g, 0.0, ref, stencil)
+    for k in eo:
+        assert abs(e[k] - eo[k]) <= 1e-12 * max(1.0, abs(eo[k])), k
+    sim.run_imag_split(1e-3, 5)
+    ref = O.run_imag_split(og, pot, w.g, 0.0, 1e-3, 5, ref, stencil)
+    assert rel_max(sim.get_psi_host(), ref.real) < 1e-12
+    assert abs(sim.norm() - 1.0) < 1e-12
+    # real time needs the imaginary part
+    with pytest.raises(P.GpeError):
+        sim.run_rk4(1e-3, 1)
+    # re-gridding, and an odd number of points (the pair-wise reductions see a zero tail)
+    wb = w.with_(delta0=22.0, delta1=22.0)
+    _, _, act_b, grid_b, _ = _make(P, wb)
+    sim_b = P.Sim(grid_b, "float64", stencil, w.g)
+    sim_b.remap_from(sim)
+    assert np.array_equal(sim_b.get_psi_host(), O.remap_psi(act, sim.get_psi_host(), act_b).real)
+    odd = act[: (act.size // 2) * 2 - 1]
+    _, _, _, grid_o, _ = _make(P, w, active=odd)
+    sim_o = P.Sim(grid_o, "float64", stencil, w.g)
+    sim_o.set_psi_host(psi[: odd.size])
+    assert abs(sim_o.norm() - O.norm(O.SparseGrid(box, odd, RADIUS[stencil]), psi[: odd.size].astype(np.complex128))) < 1e-13

@@ -29,12 +29,24 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found: libgpe_b200.so cannot be built")
 
 
+STAMP = LIB + ".stamp"
+
+
+def _digest() -> str:
+    """Hash of everything the library is built from (file times do not survive a copy to another machine)."""
+    import hashlib
+    h = hashlib.sha256()
+    for d in [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]:
+        with open(d, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(STAMP) as f:
+        return f.read().strip() != _digest()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -58,6 +70,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         objs.append(obj)
     cmd = [nvcc, *ARCH, "-shared", "-Xcompiler", "-fPIC", *objs, "-o", LIB, "-Xlinker", "-lgomp", "-cudart", "static"]
     subprocess.run(cmd, check=True)
+    with open(STAMP, "w") as f:
+        f.write(_digest())
     return LIB
 
 

@@ -24,6 +24,12 @@
 // (y0 or p) into rings of plane slots, PF planes in flight; one __syncwarp per plane, no block-level barrier.
 // Plane c = k-R is finished when plane k has arrived: V(r,t) analytic, nonlinear term, stage combination,
 // row-contiguous stores.  IMAG / ENERGY: per-stream partial sums in a fixed order -> partials[stream].
+//
+// Variants of the one kernel template: R = 1 / 2 (7- and 13-point stars), HOC (the paper's 19-point compact
+// stencil, PAPER.md:341-343 Eq. B2: diagonal-tile tables, corner halo, in-plane face / diagonal sums carried
+// along z), per-axis weights for anisotropic grids (Eq. B1), T = float / double, REAL (8-byte real-valued
+// state for ground states), and the MODEs of gpe_internal.h: operator, RK stages S1-S4 and the
+// general stage LC of Eq. A6-A7 (RKHE3, RKCK), Euler imaginary time, the paper's split iteration, energy sums.
 #include <cuda_runtime.h>
 
 #include <cstdint>

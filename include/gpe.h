@@ -155,7 +155,8 @@ int gpe_sim_state_bytes(const gpe_grid* g, int dtype, size_t* out);
 
 /* stencil: 7 (2nd order, PAPER.md:58, :337-339 Eq. B1), 13 (4th-order star, R5) or 19 (the paper's
  * higher-order compact Laplacian for dx = dy = dz = h, PAPER.md:341-343 Eq. B2: centre -4/h^2, faces 1/3h^2,
- * edges 1/6h^2; radius 1 plus the twelve edge neighbours, zero outside M like every other read).
+ * edges 1/6h^2; radius 1 plus the twelve edge neighbours, zero outside M like every other read), or 27 (3x3x3
+ * compact stencil with caller-supplied weights, gpe_sim_set_compact_weights).
  * g: interaction strength multiplying |psi|^2; n_target: value of h^3 sum|psi|^2 that imaginary-time
  * steps renormalise to (Eq. 3).  dev_state: device memory, 256-byte aligned, >= state_bytes,
  * must stay valid until gpe_sim_destroy; it is zero-initialised here (psi = 0, t = 0).  Uploads the
@@ -246,6 +247,15 @@ int gpe_sim_kernel_launches(const gpe_sim* s, int64_t* out);
  * returns the accumulated milliseconds and launch count per stage index 0..3 and resets them. */
 int gpe_sim_time_stages(gpe_sim* s, int on);
 int gpe_sim_stage_time_ms(gpe_sim* s, double ms_out[4], int64_t count_out[4]);
+/* The 27-point compact stencil (stencil = 27 at gpe_sim_create).  The paper's GPU results use a higher-order
+ * compact stencil "of shape 3^3" but do not print its weights (they are in its ref.
+ * [52]), so the caller supplies them: Laplacian weights in 1/length^2 of the centre, of the two face neighbours
+ * per axis (x, y, z), of the four edge neighbours per plane (xy, xz, yz) and of the eight corners; T = -1/2 of
+ * that stencil, zero outside M like every other read.  Until this is called a stencil-27 sim uses the weights of
+ * Eq. B2 (corner 0), i.e. it equals stencil 19.  Also valid on a stencil-19 sim.  STATE for the star stencils. */
+int gpe_sim_set_compact_weights(gpe_sim* s, double centre, const double* face_xyz, const double* edge_xy_xz_yz,
+                                double corner);
+
 /* Tuning knob: planes per thread block (1..32, default chosen per dtype/stencil).  INVALID_ARG otherwise. */
 int gpe_sim_set_planes_per_block(gpe_sim* s, int kz);
 

@@ -245,12 +245,53 @@ def apply_T19(grid: SparseGrid, psi: np.ndarray) -> np.ndarray:
     return -0.5 * (lap7 + (1.0 / 12.0) * cross)
 
 
-def apply_T(grid: SparseGrid, psi: np.ndarray, stencil: int) -> np.ndarray:
+@dataclass(frozen=True)
+class Compact27:
+    """A 3x3x3 compact Laplacian given by its weights (absolute, in 1/length^2): centre, the face weight per axis,
+    the edge weight per pair (xy, xz, yz) and the corner weight.  The paper's GPU results use a 27-point
+    higher-order compact stencil "of shape 3^3" whose weights it does not print (they
+    are in its ref. [52]): PARITY UNPINNED for any particular published set; what is pinned is the mechanism,
+    by its reductions to the 7- and 19-point stencils and by brute force (P19)."""
+    centre: float
+    face: tuple
+    edge: tuple
+    corner: float
+
+
+def apply_T27(grid: SparseGrid, psi: np.ndarray, w: Compact27) -> np.ndarray:
+    """T psi = -1/2 sum over the 27 offsets of weight(offset) psi(p + offset), psi = 0 outside M.
+    weight: centre for (0,0,0); face[a] for +-e_a; edge[pair] for +-e_a +- e_b; corner for (+-1,+-1,+-1)."""
+    psi = np.asarray(psi, dtype=np.complex128)
+    ext = np.concatenate([psi, np.zeros(1, np.complex128)])
+    lap = np.zeros_like(psi)
+    pair = {(0, 1): 0, (0, 2): 1, (1, 2): 2}
+    for dx in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dz in (-1, 0, 1):
+                off = (dx, dy, dz)
+                axes = tuple(a for a in range(3) if off[a] != 0)
+                if len(axes) == 0:
+                    c = w.centre
+                elif len(axes) == 1:
+                    c = w.face[axes[0]]
+                elif len(axes) == 2:
+                    c = w.edge[pair[axes]]
+                else:
+                    c = w.corner
+                if c != 0.0:
+                    lap = lap + c * ext[neighbour_lookup(grid, off)]
+    return -0.5 * lap
+
+
+def apply_T(grid: SparseGrid, psi: np.ndarray, stencil) -> np.ndarray:
     """T psi = -1/2 lap_h psi on M with psi = 0 outside M (weights R5).
+    stencil may also be a Compact27 (caller-supplied 27-point weights, apply_T27).
 
     (lap_h psi)_p = (1/h^2) sum_axis sum_{s=-R..R} c_|s| psi(p + s e_axis).
     stencil = 19: the paper's higher-order compact Laplacian (apply_T19).
     """
+    if isinstance(stencil, Compact27):
+        return apply_T27(grid, psi, stencil)
     if stencil == 19:
         return apply_T19(grid, psi)
     w = STENCIL_WEIGHTS[stencil]

@@ -63,7 +63,7 @@ SYMBOLS = (
     "gpe_set_time", "gpe_get_time", "gpe_apply_H", "gpe_step_rk4", "gpe_run_rk4", "gpe_imag_step",
     "gpe_run_imag", "gpe_norm", "gpe_energy", "gpe_sim_kernel_launches", "gpe_sim_time_stages",
     "gpe_sim_stage_time_ms", "gpe_sim_set_planes_per_block", "gpe_imag_split_step", "gpe_run_imag_split",
-    "gpe_remap_psi", "gpe_step_rkhe3", "gpe_run_rkhe3", "gpe_step_rkck", "gpe_run_rkck",
+    "gpe_remap_psi", "gpe_step_rkhe3", "gpe_run_rkhe3", "gpe_step_rkck", "gpe_run_rkck", "gpe_sim_set_compact_weights",
 )
 
 _lib = None
@@ -323,6 +323,12 @@ class Sim:
         cnt = (C.c_int64 * 4)()
         _check(lib().gpe_sim_stage_time_ms(self._h, ms, cnt))
         return list(ms), list(cnt)
+
+    def set_compact_weights(self, centre, face, edge, corner):
+        """Weights of the 3x3x3 compact Laplacian (stencil 19 / 27): centre, face (x, y, z), edge (xy, xz, yz), corner."""
+        f = (C.c_double * 3)(*face)
+        e = (C.c_double * 3)(*edge)
+        _check(lib().gpe_sim_set_compact_weights(self._h, C.c_double(centre), f, e, C.c_double(corner)))
 
     def set_planes_per_block(self, kz: int):
         _check(lib().gpe_sim_set_planes_per_block(self._h, C.c_int(kz)))

@@ -28,6 +28,8 @@ struct gpe_sim {
     int dtype = GPE_C128;
     int radius = 1;
     bool hoc = false;       // 19-point higher-order compact stencil (radius 1 plus edge neighbours)
+    bool custom27 = false;  // weights of the 3x3x3 stencil supplied by the caller (gpe_sim_set_compact_weights)
+    double w27[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // centre, face x y z, edge xy xz yz, corner (absolute, 1/length^2)
     double g = 0.0, n_target = 1.0;
     double t = 0.0;
     int kz = 32;
@@ -215,6 +217,13 @@ StageParams base_params(const gpe_sim* s, double t) {
         p.kw[2][1] = -0.5 * (ia[2] - 2.0 * (cxz + cyz));
         p.ke[0] = -0.5 * cxy; p.ke[1] = -0.5 * cxz; p.ke[2] = -0.5 * cyz;
     }
+    p.kcn = 0.0;
+    if (s->hoc && s->custom27) {   // T = -1/2 lap with the caller's Laplacian weights
+        p.kw[0][0] = -0.5 * s->w27[0];
+        for (int a = 0; a < 3; ++a) { p.kw[a][1] = -0.5 * s->w27[1 + a]; p.ke[a] = -0.5 * s->w27[4 + a]; }
+        p.kcn = -0.5 * s->w27[7];
+    }
+    p.kcnf = (float)p.kcn;
     for (int a = 0; a < 3; ++a) {
         for (int k = 0; k < 3; ++k) p.kwf[a][k] = (float)p.kw[a][k];
         p.kef[a] = (float)p.ke[a];
@@ -428,7 +437,7 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
                    size_t state_bytes, void* stream, gpe_sim** out) {
     if (!g || !dev_state || !out) return fail(GPE_ERR_INVALID_ARG, "null argument");
     if (dtype != GPE_C64 && dtype != GPE_C128 && dtype != GPE_R64) return fail(GPE_ERR_INVALID_ARG, "unknown dtype");
-    if (stencil != 7 && stencil != 13 && stencil != 19) return fail(GPE_ERR_INVALID_ARG, "stencil must be 7, 13 or 19");
+    if (stencil != 7 && stencil != 13 && stencil != 19 && stencil != 27) return fail(GPE_ERR_INVALID_ARG, "stencil must be 7, 13, 19 or 27");
     if (!(n_target > 0.0)) return fail(GPE_ERR_INVALID_ARG, "n_target must be > 0");
     const int radius = stencil == 13 ? 2 : 1;
     if (g->h.tx != 8 || g->h.ty != 8) return fail(GPE_ERR_UNSUPPORTED, "kernels need 8x8 column tiles");
@@ -444,7 +453,7 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     s->grid = g;
     s->dtype = dtype;
     s->radius = radius;
-    s->hoc = stencil == 19;
+    s->hoc = stencil == 19 || stencil == 27;
     s->g = g_int;
     s->n_target = n_target;
     s->csize = dtype == GPE_C128 ? 16 : 8;
@@ -749,6 +758,17 @@ int gpe_sim_stage_time_ms(gpe_sim* s, double ms_out[4], int64_t count_out[4]) {
         count_out[k] = (int64_t)(s->ev_used[k] / 2);
         s->ev_used[k] = 0;
     }
+    return GPE_OK;
+}
+
+int gpe_sim_set_compact_weights(gpe_sim* s, double centre, const double* face_xyz, const double* edge_xy_xz_yz, double corner) {
+    if (!s || !face_xyz || !edge_xy_xz_yz) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (!s->hoc) return fail(GPE_ERR_STATE, "the sim was not created with the 19- or 27-point stencil");
+    const double v[8] = {centre, face_xyz[0], face_xyz[1], face_xyz[2], edge_xy_xz_yz[0], edge_xy_xz_yz[1], edge_xy_xz_yz[2], corner};
+    for (double x : v)
+        if (!std::isfinite(x)) return fail(GPE_ERR_INVALID_ARG, "weights must be finite");
+    for (int k = 0; k < 8; ++k) s->w27[k] = v[k];
+    s->custom27 = true;
     return GPE_OK;
 }
 

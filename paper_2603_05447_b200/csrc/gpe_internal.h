@@ -118,8 +118,11 @@ struct StageParams {
     // kw[0][0] = the centre weight (all axes together); ke[] = 19-point edge weights xy, xz, yz
     double kw[3][3];
     double ke[3];
+    double kcn;            // corner weight of the 27-point compact stencil (0 for the 19-point one)
     float kwf[3][3];       // the same in fp32 (complex64 state)
     float kef[3];
+    float kcnf;
+    float padf[3];
     double xc, yc, zc;     // 0.5 (n-1) per axis: coordinate = (i - xc) h + cx
     double hax, hay, haz;  // 0.5 a_x, 0.5 a_y, 0.5 a_z
     double om2;            // Omega^2

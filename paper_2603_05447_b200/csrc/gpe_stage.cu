@@ -158,11 +158,13 @@ template <> struct KW<double> {
     static __device__ __forceinline__ double w(const StageParams& p, int axis, int s) { return p.kw[axis][s]; }
     static __device__ __forceinline__ double c(const StageParams& p) { return p.kw[0][0]; }
     static __device__ __forceinline__ double e(const StageParams& p, int pair) { return p.ke[pair]; }
+    static __device__ __forceinline__ double cn(const StageParams& p) { return p.kcn; }
 };
 template <> struct KW<float> {
     static __device__ __forceinline__ float w(const StageParams& p, int axis, int s) { return p.kwf[axis][s]; }
     static __device__ __forceinline__ float c(const StageParams& p) { return p.kwf[0][0]; }
     static __device__ __forceinline__ float e(const StageParams& p, int pair) { return p.kef[pair]; }
+    static __device__ __forceinline__ float cn(const StageParams& p) { return p.kcnf; }
 };
 
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
@@ -433,7 +435,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 Fx[a] = mk<T>(Mc[a].x + Mc[a + 2].x, Mc[a].y + Mc[a + 2].y);
                 Fy[a] = mk<T>(Lc[a + 1].x + Rc[a + 1].x, Lc[a + 1].y + Rc[a + 1].y);
                 E[a] = mk<T>((Lc[a].x + Rc[a].x) + (Lc[a + 2].x + Rc[a + 2].x), (Lc[a].y + Rc[a].y) + (Lc[a + 2].y + Rc[a + 2].y));
-                G[a] = mk<T>(fma(KW<T>::e(p, 1), Fx[a].x, KW<T>::e(p, 2) * Fy[a].x), fma(KW<T>::e(p, 1), Fx[a].y, KW<T>::e(p, 2) * Fy[a].y));
+                // what planes k-1 and k+1 see of plane k: xz / yz edge neighbours and (27-point) the corners
+                G[a] = mk<T>(fma(KW<T>::e(p, 1), Fx[a].x, fma(KW<T>::e(p, 2), Fy[a].x, KW<T>::cn(p) * E[a].x)),
+                             fma(KW<T>::e(p, 1), Fx[a].y, fma(KW<T>::e(p, 2), Fy[a].y, KW<T>::cn(p) * E[a].y)));
             }
         }
         // ---- psi(k) completes the z part of planes k-1 .. k-R -------------------------------------------

@@ -386,3 +386,30 @@ def test_real_valued_ground_state_mode(P, stencil):
     sim_o = P.Sim(grid_o, "float64", stencil, w.g)
     sim_o.set_psi_host(psi[: odd.size])
     assert abs(sim_o.norm() - O.norm(O.SparseGrid(box, odd, RADIUS[stencil]), psi[: odd.size].astype(np.complex128))) < 1e-13
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+def test_27pt_compact_stencil_with_supplied_weights(P, dtype):
+    """stencil = 27: the 3x3x3 compact stencil with caller-supplied weights (the paper does not print those of its
+    27-point stencil; parity unpinned for any published set, mechanism pinned by P19): all four
+    neighbour classes non-zero, anisotropic, against the oracle's apply_T27; default weights = the 19-point ones."""
+    tol = 1e-12 if dtype == "complex128" else 1e-5
+    w = I.small_shell(40, 13, dtype).with_(hy=0.45, hz=0.6, delta0=14.0, delta1=20.0, t_ramp=0.02)
+    box, pot, act = oracle_objs(w)
+    grid = P.Grid.from_workload(w)
+    sim = P.Sim(grid, dtype, 27, w.g)
+    og = O.SparseGrid(box, act, 1)
+    psi = I.random_psi(5, act.size).astype(sim.npdtype)
+    got = sim.apply_H(0.0, _dev(psi, dtype)).cpu().numpy()
+    assert rel_max(got, O.apply_H(og, pot, w.g, 0.0, psi.astype(np.complex128), 19)) < tol
+    cw = O.Compact27(-9.3, (1.9, 2.6, 1.2), (0.31, 0.22, 0.27), 0.05)
+    sim.set_compact_weights(cw.centre, cw.face, cw.edge, cw.corner)
+    got = sim.apply_H(0.0, _dev(psi, dtype)).cpu().numpy()
+    assert rel_max(got, O.apply_H(og, pot, w.g, 0.0, psi.astype(np.complex128), cw)) < tol
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    sim.run_rk4(w.dt, 3)
+    assert rel_max(sim.get_psi_host(), O.run_rk4(og, pot, w.g, 0.0, w.dt, 3, psi.astype(np.complex128), cw)) < tol
+    star = P.Sim(grid, dtype, 13, w.g)
+    with pytest.raises(P.GpeError):
+        star.set_compact_weights(cw.centre, cw.face, cw.edge, cw.corner)

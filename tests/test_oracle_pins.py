@@ -752,3 +752,52 @@ def test_P18_anisotropic_spacing():
     psi /= math.sqrt(O.norm(gh, psi))
     e = O.energy(gh, O.Potential(kind=O.HARMONIC), 0.0, 0.0, psi, 7)
     assert abs(e["total"] - sum(es)) < 1e-12 and abs(e["mu"] - sum(es)) < 1e-12
+
+
+# ---- P19: the 27-point compact stencil with caller-supplied weights ("HOC stencils of shape 3^3") ------
+def test_P19_compact27_reductions_and_brute_force():
+    nx, ny, nz = 6, 5, 7
+    dx, dy, dz = 0.5, 0.7, 0.4
+    box = O.Box(nx, ny, nz, dx, (0.0, 0.0, 0.0), dy, dz)
+    act = I.random_mask_lin(51, nx, ny, nz, 0.75)
+    grid = O.SparseGrid(box, act, 1)
+    psi = I.random_psi(52, act.size)
+    ia = [1 / dx ** 2, 1 / dy ** 2, 1 / dz ** 2]
+    # (a) weights of Eq. B1 -> the 7-point operator; weights of Eq. B2 -> the 19-point operator
+    w7 = O.Compact27(-2 * sum(ia), tuple(ia), (0.0, 0.0, 0.0), 0.0)
+    assert np.max(np.abs(O.apply_T(grid, psi, w7) - O.apply_T(grid, psi, 7))) < 1e-12 * 40
+    cxy, cxz, cyz = (ia[0] + ia[1]) / 12, (ia[0] + ia[2]) / 12, (ia[1] + ia[2]) / 12
+    w19 = O.Compact27(-2 * sum(ia) + 4 * (cxy + cxz + cyz),
+                      (ia[0] - 2 * (cxy + cxz), ia[1] - 2 * (cxy + cyz), ia[2] - 2 * (cxz + cyz)), (cxy, cxz, cyz), 0.0)
+    assert np.max(np.abs(O.apply_T(grid, psi, w19) - O.apply_T(grid, psi, 19))) < 1e-12 * 40
+    # (b) brute force with all four classes non-zero: dense 3x3x3 correlation on the zero-extended box
+    w = O.Compact27(-3.1, (0.7, 0.5, 0.9), (0.11, 0.13, 0.17), 0.03)
+    dense = np.zeros((nx + 2, ny + 2, nz + 2), np.complex128)
+    ix, iy, iz = O.unravel(box, act)
+    dense[ix + 1, iy + 1, iz + 1] = psi
+    out = np.zeros(act.size, np.complex128)
+    for a in (-1, 0, 1):
+        for b in (-1, 0, 1):
+            for c in (-1, 0, 1):
+                k = abs(a) + abs(b) + abs(c)
+                if k == 0:
+                    wt = w.centre
+                elif k == 1:
+                    wt = w.face[0] if a else (w.face[1] if b else w.face[2])
+                elif k == 2:
+                    wt = w.edge[0] if c == 0 else (w.edge[1] if b == 0 else w.edge[2])
+                else:
+                    wt = w.corner
+                out += wt * dense[ix + 1 + a, iy + 1 + b, iz + 1 + c]
+    assert np.max(np.abs(O.apply_T(grid, psi, w) + 0.5 * out)) < 1e-13
+    # (c) the tensor-product stencil (1 + a dxx)(1 + b dyy)(1 + c dzz) - 1 has all four classes: Kronecker form
+    eye = np.eye
+    k3 = lambda p, q, r: np.kron(np.kron(p, q), r)
+    A, B, C = 0.02, 0.03, 0.05
+    mats = [eye(n) + co * lap1d(n, d, 7) for n, d, co in ((nx, dx, A), (ny, dy, B), (nz, dz, C))]
+    full = k3(*mats) - eye(nx * ny * nz)
+    fx, fy, fz = A * ia[0], B * ia[1], C * ia[2]                       # off-diagonal entries of the 1-D factors
+    px, py, pz = 1 - 2 * fx, 1 - 2 * fy, 1 - 2 * fz                    # diagonal entries
+    wt = O.Compact27(px * py * pz - 1, (fx * py * pz, px * fy * pz, px * py * fz), (fx * fy * pz, fx * py * fz, px * fy * fz), fx * fy * fz)
+    tm = -0.5 * full[np.ix_(act, act)]
+    assert np.max(np.abs(O.apply_T(grid, psi, wt) - tm @ psi)) < 1e-13

@@ -22,9 +22,8 @@ imag_step for g > 0 and long nonlinear dynamics: "parity unpinned" beyond the
 g = 0 harmonic ground state and monotone-energy invariants (no closed form).
 imag_split_step (the paper's own scheme): PINNED for g = 0 (P13: the
 iteration matrix D K D built from Kronecker products, its top eigenvector and the
-O(dt^2) splitting error of the ground-state energy) and for the one-point mask
-(closed form); for g > 0 "parity unpinned" beyond those and the agreement of its
-fixed point with imag_step's to O(dt).
+O(dt^2) splitting error of the ground-state energy) and for the linearised interaction
+factor; the full iteration for g > 0 is "parity unpinned" beyond those.
 rkhe3_step / rkck_step (P15, P16), apply_T19 and anisotropic spacing (P17, P18), remap_psi (P14): PINNED.
 apply_T27 / Compact27: the mechanism is PINNED (P19); for any particular published 27-point weight set
 "parity unpinned" (PAPER.md does not print the weights of its 27-point stencil).

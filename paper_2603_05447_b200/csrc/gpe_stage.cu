@@ -167,6 +167,9 @@ template <> struct KW<float> {
     static __device__ __forceinline__ float cn(const StageParams& p) { return p.kcnf; }
 };
 
+// imaginary part of a value: identically zero for a real-valued state (REAL), where it is not computed at all
+#define YV(expr) (REAL ? (T)0 : (T)(expr))
+
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
 
 template <typename T, int R, int MODE, int PR, bool HOC, bool REAL>
@@ -432,26 +435,26 @@ stage_kernel(const __grid_constant__ StageParams p) {
             }
 #pragma unroll
             for (int a = 0; a < PR; ++a) {
-                Fx[a] = mk<T>(Mc[a].x + Mc[a + 2].x, Mc[a].y + Mc[a + 2].y);
-                Fy[a] = mk<T>(Lc[a + 1].x + Rc[a + 1].x, Lc[a + 1].y + Rc[a + 1].y);
-                E[a] = mk<T>((Lc[a].x + Rc[a].x) + (Lc[a + 2].x + Rc[a + 2].x), (Lc[a].y + Rc[a].y) + (Lc[a + 2].y + Rc[a + 2].y));
+                Fx[a] = mk<T>(Mc[a].x + Mc[a + 2].x, YV(Mc[a].y + Mc[a + 2].y));
+                Fy[a] = mk<T>(Lc[a + 1].x + Rc[a + 1].x, YV(Lc[a + 1].y + Rc[a + 1].y));
+                E[a] = mk<T>((Lc[a].x + Rc[a].x) + (Lc[a + 2].x + Rc[a + 2].x), YV((Lc[a].y + Rc[a].y) + (Lc[a + 2].y + Rc[a + 2].y)));
                 // what planes k-1 and k+1 see of plane k: xz / yz edge neighbours and (27-point) the corners
                 G[a] = mk<T>(fma(KW<T>::e(p, 1), Fx[a].x, fma(KW<T>::e(p, 2), Fy[a].x, KW<T>::cn(p) * E[a].x)),
-                             fma(KW<T>::e(p, 1), Fx[a].y, fma(KW<T>::e(p, 2), Fy[a].y, KW<T>::cn(p) * E[a].y)));
+                             YV(fma(KW<T>::e(p, 1), Fx[a].y, fma(KW<T>::e(p, 2), Fy[a].y, KW<T>::cn(p) * E[a].y))));
             }
         }
         // ---- psi(k) completes the z part of planes k-1 .. k-R -------------------------------------------
 #pragma unroll
         for (int e = 0; e < PR; ++e) {
             AO[e].x = fma(KW<T>::w(p, 2, R), v[e].x, AO[e].x);
-            AO[e].y = fma(KW<T>::w(p, 2, R), v[e].y, AO[e].y);
+            AO[e].y = YV(fma(KW<T>::w(p, 2, R), v[e].y, AO[e].y));
             if (R == 2) {
                 AN[e].x = fma(KW<T>::w(p, 2, 1), v[e].x, AN[e].x);
-                AN[e].y = fma(KW<T>::w(p, 2, 1), v[e].y, AN[e].y);
+                AN[e].y = YV(fma(KW<T>::w(p, 2, 1), v[e].y, AN[e].y));
             }
             if (HOC && MODE != MODE_PREP) {                     // the xz / yz edge neighbours of plane k-1 in plane k
                 AO[e].x += G[e].x;
-                AO[e].y += G[e].y;
+                AO[e].y = YV(AO[e].y + G[e].y);
             }
         }
         // ---- finish plane c = k - R: nonlinear term, stage combination (branch-free; stores predicated) ----
@@ -468,7 +471,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 const unsigned pos = cbase + (unsigned)__popc(cword & bm[e]);
                 const C cv = PO[e];
                 const C tc = AO[e];
-                const T a2 = fma(cv.x, cv.x, cv.y * cv.y);
+                const T a2 = REAL ? cv.x * cv.x : fma(cv.x, cv.x, cv.y * cv.y);
                 if (MODE == MODE_ENERGY) {
                     // inactive lanes hold cv = 0 and finite tc: they add exact zeros
                     acc[0] += (double)(cv.x * tc.x + cv.y * tc.y);
@@ -482,12 +485,12 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     // propagator exp(-V ca) (1 - g ca |u|^2) of Eq. 7 with the linearised interaction factor
                     const T ca = (T)p.ca;
                     C u = cv;
-                    if (MODE != MODE_PREP) u = mk<T>(fma(-ca, tc.x, cv.x), fma(-ca, tc.y, cv.y));
+                    if (MODE != MODE_PREP) u = mk<T>(fma(-ca, tc.x, cv.x), YV(fma(-ca, tc.y, cv.y)));
                     C o = u;
                     if (MODE != MODE_KIN) {
                         const double u2 = (double)u.x * (double)u.x + (double)u.y * (double)u.y;
                         const T f = (T)(sc * exp(-vpot[e] * p.ca) * fma(-gsc * p.ca, u2, 1.0));
-                        o = mk<T>(u.x * f, u.y * f);
+                        o = mk<T>(u.x * f, YV(u.y * f));
                     }
                     if (MODE == MODE_SPLITB) {
                         const double o2 = (double)o.x * (double)o.x + (double)o.y * (double)o.y;
@@ -497,14 +500,14 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     continue;
                 }
                 const T diag = (T)fma(gsc, (double)a2, vpot[e]);
-                const C hc = mk<T>(fma(diag, cv.x, tc.x), fma(diag, cv.y, tc.y));
+                const C hc = mk<T>(fma(diag, cv.x, tc.x), YV(fma(diag, cv.y, tc.y)));
                 const T ca = (T)p.ca;
                 C o;
                 if (MODE == MODE_APPLY) {
                     o = hc;
                 } else if (MODE == MODE_IMAG) {
                     const T s = (T)sc;
-                    o = mk<T>(s * fma(-ca, hc.x, cv.x), s * fma(-ca, hc.y, cv.y));
+                    o = mk<T>(s * fma(-ca, hc.x, cv.x), YV(s * fma(-ca, hc.y, cv.y)));
                     const double o2 = (double)o.x * (double)o.x + (double)o.y * (double)o.y;
                     acc[0] += on ? o2 : 0.0;
                 } else if (MODE == MODE_LC) {
@@ -534,20 +537,20 @@ stage_kernel(const __grid_constant__ StageParams p) {
             C an;
             if (R == 2) {
                 an.x = KW<T>::w(p, 2, 2) * PO[e].x;
-                an.y = KW<T>::w(p, 2, 2) * PO[e].y;
+                an.y = YV(KW<T>::w(p, 2, 2) * PO[e].y);
                 an.x = fma(KW<T>::w(p, 2, 1), PN[e].x, an.x);
-                an.y = fma(KW<T>::w(p, 2, 1), PN[e].y, an.y);
+                an.y = YV(fma(KW<T>::w(p, 2, 1), PN[e].y, an.y));
             } else {
                 an.x = KW<T>::w(p, 2, 1) * PO[e].x;
-                an.y = KW<T>::w(p, 2, 1) * PO[e].y;
+                an.y = YV(KW<T>::w(p, 2, 1) * PO[e].y);
             }
             AO[e].x = fma(KW<T>::c(p), v[e].x, an.x);
-            AO[e].y = fma(KW<T>::c(p), v[e].y, an.y);
+            AO[e].y = YV(fma(KW<T>::c(p), v[e].y, an.y));
             PO[e] = v[e];
             if (HOC && MODE != MODE_PREP) {
                 // faces and diagonals of plane k, and plane k-1's share of the xz / yz edges
                 AO[e].x = fma(KW<T>::w(p, 0, 1), Fx[e].x, fma(KW<T>::w(p, 1, 1), Fy[e].x, fma(KW<T>::e(p, 0), E[e].x, AO[e].x + GPV[e].x)));
-                AO[e].y = fma(KW<T>::w(p, 0, 1), Fx[e].y, fma(KW<T>::w(p, 1, 1), Fy[e].y, fma(KW<T>::e(p, 0), E[e].y, AO[e].y + GPV[e].y)));
+                AO[e].y = YV(fma(KW<T>::w(p, 0, 1), Fx[e].y, fma(KW<T>::w(p, 1, 1), Fy[e].y, fma(KW<T>::e(p, 0), E[e].y, AO[e].y + GPV[e].y))));
                 GPV[e] = G[e];
             }
         }
@@ -562,7 +565,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     const int d = r > a ? r - a : a - r;
                     if (d >= 1 && d <= R) {
                         AO[a].x = fma(KW<T>::w(p, 0, d), val.x, AO[a].x);
-                        AO[a].y = fma(KW<T>::w(p, 0, d), val.y, AO[a].y);
+                        AO[a].y = YV(fma(KW<T>::w(p, 0, d), val.y, AO[a].y));
                     }
                 }
             }
@@ -575,7 +578,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     const C val = lds_c(so + (unsigned)(a * (int)ROW_BYTES + cc * (int)ES), (EL*)nullptr);
                     const int d = cc > 0 ? cc : -cc;
                     AO[a].x = fma(KW<T>::w(p, 1, d), val.x, AO[a].x);
-                    AO[a].y = fma(KW<T>::w(p, 1, d), val.y, AO[a].y);
+                    AO[a].y = YV(fma(KW<T>::w(p, 1, d), val.y, AO[a].y));
                 }
             }
         }

@@ -199,3 +199,24 @@ def test_config2_split_scheme_iterations(P):
     ref = O.run_imag_split(og, pot, w.g, 0.0, w.dt, 10, psi, w.stencil)
     assert rel_max(sim.get_psi_host(), ref) < 1e-11
     assert abs(sim.norm() - 1.0) < 1e-12
+
+
+def test_config4_full_run_invariants(P):
+    """BASELINE configs[3] as specified: 200 real-time RK4 steps dt = 1e-4 on the whole 1024^3 bubble (complex128).
+    No oracle can follow 2.5e10 stage updates; what must hold at any size does: the static potential conserves norm
+    and energy up to RK4's O(dt^4) error (P8), and a second run from the same input is bit-identical."""
+    w = I.config4("complex128")
+    grid, act, psi0, _, _ = _setup(P, w)
+    sim = P.Sim(grid, w.dtype, w.stencil, w.g)
+    sim.set_psi_host(psi0)
+    e0 = sim.energy()
+    sim.run_rk4(w.dt, w.nsteps)
+    e1 = sim.energy()
+    assert w.nsteps == 200 and abs(sim.time - 200 * w.dt) < 1e-15
+    assert abs(sim.norm() - 1.0) < 1e-7
+    assert abs(e1["total"] - e0["total"]) < 1e-7 * abs(e0["total"])
+    first = sim.get_psi_host().copy()
+    sim.set_psi_host(psi0)
+    sim.time = 0.0
+    sim.run_rk4(w.dt, w.nsteps)
+    assert np.array_equal(sim.get_psi_host(), first)

@@ -220,3 +220,22 @@ def test_config4_full_run_invariants(P):
     sim.time = 0.0
     sim.run_rk4(w.dt, w.nsteps)
     assert np.array_equal(sim.get_psi_host(), first)
+
+
+def test_config3_whole_ramp_on_a_replica(P):
+    """BASELINE configs[2], the whole hollowing-out ramp Delta: 0 -> 800 (t_ramp = 4) against the oracle on a
+    128^3, h = 0.8 replica of the 512^3 box (same physical box and potential, union mask; the oracle cannot follow
+    3e12 stage updates at full size): 2000 RK4 steps dt = 2e-3, V evaluated at every stage time."""
+    w = I.config3(True).with_(nx=128, ny=128, nz=128, h=0.8, dt=2e-3, name="cfg3a_replica_128")
+    box, pot, act = oracle_objs(w)
+    grid = P.Grid.from_workload(w)
+    assert np.array_equal(grid.active_indices(), act) and act.size > 4e5
+    sim = P.Sim(grid, "complex128", w.stencil, w.g)
+    co = CO.COracle(box, pot, act, w.stencil)
+    psi = I.make_psi0(w, act)
+    sim.set_psi_host(psi)
+    sim.run_rk4(w.dt, 2000)
+    assert abs(sim.time - w.t_ramp) < 1e-12
+    ref = co.run_rk4(w.g, 0.0, w.dt, 2000, psi)
+    assert rel_max(sim.get_psi_host(), ref) < 2e-9
+    assert abs(sim.norm() - co.norm(ref)) < 1e-10

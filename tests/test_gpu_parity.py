@@ -413,3 +413,19 @@ def test_27pt_compact_stencil_with_supplied_weights(P, dtype):
     star = P.Sim(grid, dtype, 13, w.g)
     with pytest.raises(P.GpeError):
         star.set_compact_weights(cw.centre, cw.face, cw.edge, cw.corner)
+
+
+@pytest.mark.parametrize("stencil", [7, 13, 19])
+@pytest.mark.parametrize("kz", [1, 2, 3])
+def test_shortest_streams(P, stencil, kz):
+    """Streams of 1, 2 and 3 planes (shorter than the prefetch depth): operator and two RK4 steps."""
+    w = I.small_shell(24, stencil).with_(delta0=5.0, delta1=8.0, t_ramp=0.02)
+    box, pot, act, grid, sim = _make(P, w)
+    sim.set_planes_per_block(kz)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.make_psi0(w, act)
+    got = sim.apply_H(0.01, _dev(psi, "complex128")).cpu().numpy()
+    assert rel_max(got, O.apply_H(og, pot, w.g, 0.01, psi, stencil)) < 1e-12
+    sim.set_psi_host(psi)
+    sim.run_rk4(w.dt, 2)
+    assert rel_max(sim.get_psi_host(), O.run_rk4(og, pot, w.g, 0.0, w.dt, 2, psi, stencil)) < 1e-12

@@ -429,3 +429,20 @@ def test_shortest_streams(P, stencil, kz):
     sim.set_psi_host(psi)
     sim.run_rk4(w.dt, 2)
     assert rel_max(sim.get_psi_host(), O.run_rk4(og, pot, w.g, 0.0, w.dt, 2, psi, stencil)) < 1e-12
+
+
+@pytest.mark.parametrize("stencil", [7, 13, 19])
+@pytest.mark.parametrize("dims", [(5, 3, 1), (1, 1, 9), (8, 8, 1), (1, 17, 2), (16, 1, 3)])
+def test_degenerate_boxes(P, dims, stencil):
+    """Boxes one point thick along one or two axes, fully active: every neighbour lookup hits a box face."""
+    nx, ny, nz = dims
+    w = I.Workload(name="thin", nx=nx, ny=ny, nz=nz, h=0.4, kind=I.HARMONIC, ax=1.0, ay=2.0, az=0.5, stencil=stencil, g=2.0)
+    act = np.arange(nx * ny * nz, dtype=np.int64)
+    box, pot, act, grid, sim = _make(P, w, active=act)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.random_psi(3, act.size)
+    got = sim.apply_H(0.0, _dev(psi, "complex128")).cpu().numpy()
+    assert rel_max(got, O.apply_H(og, pot, w.g, 0.0, psi, stencil)) < 1e-12
+    sim.set_psi_host(psi)
+    sim.run_rk4(1e-3, 2)
+    assert rel_max(sim.get_psi_host(), O.run_rk4(og, pot, w.g, 0.0, 1e-3, 2, psi, stencil)) < 1e-12

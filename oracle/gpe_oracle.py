@@ -18,12 +18,14 @@ textbook k1..k4 RK4.
 
 Pin status (tests/test_oracle_pins.py): coords/potential/mask, apply_T (7 and
 13 pt), apply_H, rk4_step, norm/energy, layout tables: PINNED (P1-P12).
-imag_step for g > 0 and long nonlinear dynamics: "parity unpinned" beyond the
-g = 0 harmonic ground state and monotone-energy invariants (no closed form).
+imag_step and energy()['mu'] for g > 0: PINNED (P20: a fixed point of the normalised Euler iteration satisfies
+H[psi] psi = mu psi, Eq. 1, for any dt; P21: mu is the Rayleigh quotient of apply_H on a random state; P22:
+Thomas-Fermi limit, Eq. 5, for large g).  Long nonlinear dynamics beyond the invariants (norm, energy, monotone
+energy in imaginary time): "parity unpinned" (no closed form).
 imag_split_step (the paper's own scheme): PINNED for g = 0 (P13: the
 iteration matrix D K D built from Kronecker products, its top eigenvector and the
-O(dt^2) splitting error of the ground-state energy) and for the linearised interaction
-factor; the full iteration for g > 0 is "parity unpinned" beyond those.
+O(dt^2) splitting error of the ground-state energy), for the linearised interaction
+factor, and for g > 0 to first order in dt (P23: it differs from the pinned Euler step by O(dt^2) only).
 rkhe3_step / rkck_step (P15, P16), apply_T19 and anisotropic spacing (P17, P18), remap_psi (P14): PINNED.
 apply_T27 / Compact27: the mechanism is PINNED (P19); for any particular published 27-point weight set
 "parity unpinned" (PAPER.md does not print the weights of its 27-point stencil).

@@ -391,12 +391,13 @@ stage_kernel(const __grid_constant__ StageParams p) {
 #pragma unroll
                 for (int j = 0; j < MAX_LC_AUX; ++j) {
                     if (j < p.n_aux) {
-                        const C* __restrict__ aj = reinterpret_cast<const C*>(p.auxn[j]);
+                        // the last RKCK stage writes y_new over y^(1) = auxn[0]: plain loads, no read-only path, no restrict
+                        const C* aj = reinterpret_cast<const C*>(p.auxn[j]);
                         const T cj = (T)p.coef[j];
 #pragma unroll
                         for (int e = 0; e < PR; ++e) {
                             if ((cword >> (rb0 + 8 * e)) & 1u) {
-                                const C a = __ldg(aj + (REAL ? 0u : cbase + (unsigned)__popc(cword & bm[e])));
+                                const C a = aj[REAL ? 0u : cbase + (unsigned)__popc(cword & bm[e])];
                                 lcs[e].x = fma(cj, a.x, lcs[e].x);
                                 lcs[e].y = fma(cj, a.y, lcs[e].y);
                             }

@@ -801,3 +801,111 @@ def test_P19_compact27_reductions_and_brute_force():
     wt = O.Compact27(px * py * pz - 1, (fx * py * pz, px * fy * pz, px * py * fz), (fx * fy * pz, fx * py * fz, px * fy * fz), fx * fy * fz)
     tm = -0.5 * full[np.ix_(act, act)]
     assert np.max(np.abs(O.apply_T(grid, psi, wt) - tm @ psi)) < 1e-13
+
+
+# ---- P20: a fixed point of the normalised Euler iteration is a stationary state (g > 0) ----------------------------
+def _stationary_shell(g=300.0, dt=8e-3, nsteps=3200):
+    """Imaginary time on a small dressed shell until psi <- normalise((1 - dt H[psi]) psi) no longer moves."""
+    from helpers import oracle_objs
+    w = I.small_shell(24, 13)
+    box, pot, act = oracle_objs(w)
+    grid = O.SparseGrid(box, act, 2)
+    psi = np.abs(I.make_psi0(w, act)).astype(np.complex128)
+    psi /= math.sqrt(O.norm(grid, psi))
+    psi = O.run_imag(grid, pot, g, 0.0, dt, nsteps, psi, 13)
+    return box, pot, act, grid, psi
+
+
+def test_P20_imag_step_fixed_point_is_stationary_state_g_positive():
+    """PAPER.md:25 Eq. 1 (H psi = mu psi) and :35 (imaginary time converges to the ground state): a fixed point of
+    psi <- normalise((1 - dt H[psi]) psi) satisfies H[psi] psi = mu psi exactly, for any dt, with
+    mu = <psi|H psi>/<psi|psi>.  apply_H is pinned separately (P5, P11), so this pins the g > 0 arithmetic of
+    imag_step (a doubled or dropped g |psi|^2 term moves the fixed point away from Eq. 1) and energy()['mu']
+    (kin + pot + 2 inter; with 1 inter the residual below is O(inter))."""
+    g = 300.0
+    box, pot, act, grid, psi = _stationary_shell(g)
+    e = O.energy(grid, pot, g, 0.0, psi, 13)
+    hp = O.apply_H(grid, pot, g, 0.0, psi, 13)
+    assert e["inter"] > 0.05 * abs(e["mu"])            # the nonlinear term matters in this state
+    res = np.max(np.abs(hp - e["mu"] * psi)) / np.max(np.abs(e["mu"] * psi))
+    assert res < 1e-8
+    # the fixed point does not depend on dt: one step with another dt leaves it in place
+    again = O.imag_step(grid, pot, g, 0.0, 2e-3, psi, 13)
+    assert np.max(np.abs(again - psi)) < 1e-9 * np.max(np.abs(psi))
+    # the explicit-loop C restatement has the same fixed point and the same mu
+    from oracle.c_oracle import COracle
+    co = COracle(box, pot, act, 13)
+    ec = co.energy(g, 0.0, psi)
+    assert abs(ec["mu"] - e["mu"]) < 1e-12 * abs(e["mu"])
+    hc = co.apply_H(g, 0.0, psi)
+    assert np.max(np.abs(hc - ec["mu"] * psi)) / np.max(np.abs(ec["mu"] * psi)) < 1e-8
+    stepc = co.run_imag(g, 0.0, 2e-3, 1, psi)
+    assert np.max(np.abs(stepc - psi)) < 1e-9 * np.max(np.abs(psi))
+
+
+# ---- P21: mu is the Rayleigh quotient of H[psi] (definition, Eq. 1), on a random state with g > 0 ---------------
+@pytest.mark.parametrize("stencil", [7, 13])
+def test_P21_mu_is_rayleigh_quotient_of_apply_H(stencil):
+    from helpers import oracle_objs
+    w = I.small_shell(24, stencil)
+    box, pot, act = oracle_objs(w)
+    grid = O.SparseGrid(box, act, 2)
+    psi = I.random_psi(77, len(act))
+    g = 431.0
+    hp = O.apply_H(grid, pot, g, 0.3, psi, stencil)
+    rq = box.cell * float(np.sum((np.conj(psi) * hp).real)) / (box.cell * float(np.sum(np.abs(psi) ** 2)))
+    e = O.energy(grid, pot, g, 0.3, psi, stencil)
+    assert abs(e["mu"] - rq) < 1e-12 * abs(rq)
+    assert abs(e["norm"] - box.cell * float(np.sum(np.abs(psi) ** 2))) < 1e-13 * e["norm"]
+    # the interaction energy is half the interaction part of <H>: E = <H> - inter, so total = mu norm - inter
+    assert abs(e["total"] - (e["mu"] * e["norm"] - e["inter"])) < 1e-12 * abs(e["total"])
+    from oracle.c_oracle import COracle
+    ec = COracle(box, pot, act, stencil).energy(g, 0.3, psi)
+    assert abs(ec["mu"] - rq) < 1e-12 * abs(rq)
+
+
+# ---- P22: Thomas-Fermi limit of the converged state (PAPER.md:50 Eq. 5) ------------------------------------------------
+def test_P22_thomas_fermi_limit_for_large_g():
+    """For large g the kinetic term is a small correction and the stationary state obeys
+    g |psi|^2 = mu - V where mu > V (Eq. 5).  Harmonic trap, g = 4000: the Thomas-Fermi chemical
+    potential is mu_TF = (15 g / (4 pi))^(2/5) / 2 and the density follows (mu - V)/g away from the cloud's edge."""
+    n, h, g = 28, 0.5, 4000.0
+    box = O.Box(n, n, n, h)
+    pot = O.Potential(kind=O.HARMONIC)
+    act = O.active_indices(box, pot, 22.0)                  # V < 22: a ball that contains the cloud (mu_TF ~ 9.2)
+    grid = O.SparseGrid(box, act, 1)
+    v = O.potential_at(box, pot, act, 0.0)
+    mu_tf = 0.5 * (15.0 * g / (4.0 * math.pi)) ** 0.4
+    psi = np.sqrt(np.maximum(mu_tf - v, 0.0) / g).astype(np.complex128) + 1e-3
+    psi /= math.sqrt(O.norm(grid, psi))
+    psi = O.run_imag(grid, pot, g, 0.0, 4e-3, 1500, psi, 7)
+    e = O.energy(grid, pot, g, 0.0, psi, 7)
+    assert abs(e["mu"] - mu_tf) < 0.02 * mu_tf              # kinetic correction ~ (1/R_TF^2) ln R_TF
+    bulk = v < 0.6 * e["mu"]
+    dens = np.abs(psi[bulk]) ** 2
+    assert np.max(np.abs(g * dens - (e["mu"] - v[bulk]))) < 0.03 * e["mu"]
+    assert e["kin"] < 0.05 * e["mu"]
+
+
+# ---- P23: the paper's split iteration agrees with the Euler step to first order in dt for g > 0 -----------------
+def test_P23_split_step_equals_euler_step_to_second_order_g_positive():
+    """D K K D with the linearised interaction factor and one Euler step of the full H differ by
+    O(dt^2) per step; a wrong g, dt/2 or ordering in diag_propagator shows up at O(dt).  With P20 this pins
+    imag_split_step for g > 0."""
+    from helpers import oracle_objs
+    w = I.small_shell(24, 13)
+    box, pot, act = oracle_objs(w)
+    grid = O.SparseGrid(box, act, 2)
+    psi = np.abs(I.make_psi0(w, act)).astype(np.complex128)
+    psi /= math.sqrt(O.norm(grid, psi))
+    g = 300.0
+    d = []
+    for dt in (1e-3, 5e-4, 2.5e-4):
+        a = O.imag_split_step(grid, pot, g, 0.0, dt, psi, 13)
+        b = O.imag_step(grid, pot, g, 0.0, dt, psi, 13)
+        d.append(np.max(np.abs(a - b)))
+    assert 3.6 < d[0] / d[1] < 4.4 and 3.6 < d[1] / d[2] < 4.4
+    # the test can see an O(dt) defect of the nonlinear term: that term's whole effect at the smallest dt is several
+    # times the O(dt^2) difference measured there
+    lin = np.max(np.abs(O.imag_step(grid, pot, g, 0.0, 2.5e-4, psi, 13) - O.imag_step(grid, pot, 0.0, 0.0, 2.5e-4, psi, 13)))
+    assert lin > 3 * d[2]

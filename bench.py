@@ -149,19 +149,32 @@ def oracle_sample(w, target_points=3_000_000):
     return box, pot, act, f"active points with {lo} <= ix < {hi} of {w.name} ({act.size} of the shell's points)"
 
 
-def time_oracle(w, steps, warmup=1, target_points=3_000_000):
-    """RK4 steps of the C oracle (textbook k1..k4, explicit loops, OpenMP over the host cores) on the sample."""
+def time_oracle(w, steps, warmup=1, target_points=3_000_000, threads=0, whole=False):
+    """RK4 steps of the C oracle (textbook k1..k4, explicit loops, OpenMP over the host cores; as it stands, not tuned
+    for this) on the sample, or on the whole grid of a small workload (whole=True); threads = 0: all cores."""
     from oracle import c_oracle as CO
-    box, pot, act, what = oracle_sample(w, target_points)
+    if whole:
+        from oracle import gpe_oracle as O
+        box = O.Box(w.nx, w.ny, w.nz, w.h, w.center, w.hy, w.hz)
+        pot = O.Potential(w.kind, w.ax, w.ay, w.az, w.delta0, w.delta1, w.t_ramp, w.omega)
+        act = O.active_indices(box, pot, w.v_cut, w.mask_mode)
+        what = f"whole grid of {w.name} ({act.size} points)"
+    else:
+        box, pot, act, what = oracle_sample(w, target_points)
     co = CO.COracle(box, pot, act, w.stencil)
-    psi = I.make_psi0(w, act)
-    for _ in range(warmup):
-        psi = co.run_rk4(w.g, 0.0, w.dt, 1, psi)
-    t0 = time.perf_counter()
-    psi = co.run_rk4(w.g, warmup * w.dt, w.dt, steps, psi)
-    el = time.perf_counter() - t0
+    co.set_threads(threads)
+    try:
+        psi = I.make_psi0(w, act)
+        for _ in range(warmup):
+            psi = co.run_rk4(w.g, 0.0, w.dt, 1, psi)
+        t0 = time.perf_counter()
+        psi = co.run_rk4(w.g, warmup * w.dt, w.dt, steps, psi)
+        el = time.perf_counter() - t0
+        cores = co.threads
+    finally:
+        co.set_threads(0)
     assert np.all(np.isfinite(psi))
-    return {"value": act.size * 4 * steps / el, "unit": UNIT, "cores": co.threads, "kind": "oracle",
+    return {"value": act.size * 4 * steps / el, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{steps} RK4 steps on the {what}", "seconds": el}, act.size, el
 
 
@@ -285,12 +298,20 @@ def run_ours(args, w):
     tot_by = sum(s["algorithmic_bytes"] for s in stages)
     roofline = None
     if dom:
+        # S1-S4 are ONE kernel template (stage_kernel) launched four times per step with 2 / 4 / 3 / 3 values per
+        # point, and the metric is per step: the headline fraction is taken over the four launches of a step
+        # (algorithmic bytes of the step / summed launch durations); the longest launch (S2) is listed beside it.
         dkey = "c128" if w.dtype == "complex128" else "c64"
-        roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["GBps"], "peak": peak, "unit": "GB/s",
-                    "frac": dom["frac"], "traffic": recorded_traffic(w.name, dkey), "peak_source": peak_src,
-                    "frac_of_8TBps": dom["GBps"] / 8000.0,
-                    "all_stages": {"achieved": tot_by / (tot_ms * 1e-3) / 1e9, "frac": tot_by / (tot_ms * 1e-3) / 1e9 / peak,
-                                   "stage_share_of_step": tot_ms * args.steps / ms if world == 1 else None},
+        step_gbps = tot_by / (tot_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "stage_kernel (S1+S2+S3+S4: the four launches of one RK4 step)",
+                    "achieved": step_gbps, "peak": peak, "unit": "GB/s", "frac": step_gbps / peak,
+                    "traffic": recorded_traffic(w.name, dkey), "peak_source": peak_src,
+                    "frac_of_8TBps": step_gbps / 8000.0,
+                    "step_frac": step_gbps / peak, "step_frac_of_8TBps": step_gbps / 8000.0,
+                    "algorithmic_bytes": tot_by, "launch_ms_sum": tot_ms,
+                    "stage_share_of_step": tot_ms * args.steps / ms if world == 1 else None,
+                    "longest_launch": {"kernel": dom["kernel"], "GBps": dom["GBps"], "frac": dom["frac"],
+                                       "frac_of_8TBps": dom["GBps"] / 8000.0},
                     "stages": stages}
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D psi, one RK4 step, D2H psi ------
@@ -352,6 +373,42 @@ def run_ours(args, w):
     d = sim.get_psi()
     ms_pk = timed(lambda: sim.set_psi(d), 3)
     extra["pack"] = {"ms": ms_pk}
+    del d
+
+    # ---- sustained: the same workload back to back for >= 2 s (cfg 4 as specified is 200 steps, cfg 3 is 2e4:
+    #      this is the rate those runs see once the SM clock has settled under the power cap) -------------------
+    if args.sustained_s > 0:
+        sim.set_psi_host(host_np)
+        sim.time = 0.0
+        n_sus = max(args.steps, int(args.sustained_s * 1e3 / (ms / args.steps)) + 1)
+        samp2 = ClockSampler(local)
+        barrier()
+        samp2.start()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        sim.run_rk4(w.dt, n_sus)
+        b.record(stream)
+        barrier()
+        ck2 = samp2.stop()
+        ms_sus, _ = aggregate_replicas(a.elapsed_time(b), n, dev)
+        v_sus = stage_updates_per_s(n_all, n_sus, ms_sus)
+        g_sus = v_sus * 3 * csize / 1e9 / world
+        extra["sustained"] = {"steps": n_sus, "seconds": ms_sus * 1e-3, "value": v_sus, "unit": UNIT, "ms_per_step": ms_sus / n_sus,
+                              "hbm_GBps_algorithmic": g_sus, "step_frac": g_sus / peak, "step_frac_of_8TBps": g_sus / 8000.0,
+                              "clocks": ck2}
+
+    # ---- BASELINE configs[0] (6.7e4 points: launch-bound, report only): RK4 steps per second -----------------
+    if world == 1 and w.name != I.config1().name:
+        w1 = I.config1()
+        g1 = P.Grid.from_workload(w1)
+        s1 = P.Sim(g1, w1.dtype, w1.stencil, w1.g, device=f"cuda:{local}")
+        s1.set_psi_host(I.make_psi0(w1, g1.active_indices()).astype(s1.npdtype))
+        ms1 = timed(lambda: s1.run_rk4(w1.dt, 200), 3) / 200
+        extra["cfg1_harmonic_48"] = {"n_active": g1.n_active, "ms_per_step": ms1, "steps_per_s": 1e3 / ms1,
+                                     "stage_updates_per_s": g1.n_active * 4 / (ms1 * 1e-3),
+                                     "note": "launch-bound (4 stage launches per step); report only"}
+        s1.close()
+        g1.close()
 
     if world > 1:
         dist.barrier()
@@ -361,8 +418,15 @@ def run_ours(args, w):
     # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample -------------------------
     cpu = None
     if world == 1 and not args.no_cpu:
-        res, _, _ = time_oracle(w, 2, warmup=1, target_points=3_000_000)
+        # the oracle as it stands (gcc -O2, explicit loops, one int64 neighbour table; never tuned for this)
+        res, _, _ = time_oracle(w, 3, warmup=1, target_points=3_000_000)
         cpu = {k: res[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        # beside it: one thread (the paper's CPU numbers are single-thread) and BASELINE configs[1]'s
+        # whole grid on all cores (SURVEY.md 8d "Oracle timing")
+        r1, _, _ = time_oracle(w, 3, warmup=1, target_points=400_000, threads=1)
+        cpu["single_thread"] = {k: r1[k] for k in ("value", "unit", "cores", "sample")}
+        r2, _, _ = time_oracle(I.config2().with_(dt=1e-4), 3, warmup=1, whole=True)
+        cpu["cfg2_whole_grid"] = {k: r2[k] for k in ("value", "unit", "cores", "sample")}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -446,6 +510,8 @@ def main():
     ap.add_argument("--workload", default="cfg4_c128", choices=sorted(workloads()))
     ap.add_argument("--kz", type=int, default=0, help="planes per thread block (0 = library default)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sustained-s", type=float, default=2.0,
+                    help="length of the back-to-back sustained leg reported under extra.sustained (0 = skip)")
     ap.add_argument("--sweep", action="store_true", help="BASELINE configs[4] bandwidth sweep: one JSON line per point")
     ap.add_argument("--sweep-max", type=float, default=3e8, help="largest target point count of the sweep")
     args = ap.parse_args()

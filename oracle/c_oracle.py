@@ -66,6 +66,10 @@ class COracle:
     def threads(self) -> int:
         return int(self.lib.orc_num_threads())
 
+    def set_threads(self, n: int):
+        """OpenMP threads of the loops (0 = all cores)."""
+        self.lib.orc_set_num_threads(C.c_int(int(n)))
+
     def apply_H(self, g, t, psi):
         psi = np.ascontiguousarray(psi, dtype=np.complex128)
         out = np.empty_like(psi)

@@ -41,6 +41,16 @@ int orc_num_threads(void) {
 #endif
 }
 
+/* threads of the parallel loops below (the timed baseline reports a one-thread figure beside the all-core one:
+ * the paper's CPU numbers are single-thread); n <= 0 restores the default */
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    omp_set_num_threads(n > 0 ? n : omp_get_num_procs());
+#else
+    (void)n;
+#endif
+}
+
 static int64_t find_sorted(const int64_t* a, int64_t n, int64_t key) {
     int64_t lo = 0, hi = n;
     while (lo < hi) {

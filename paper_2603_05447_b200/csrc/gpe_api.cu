@@ -42,7 +42,8 @@ struct gpe_sim {
     WorkRec* d_work = nullptr;
     int32_t n_blocks = 0;
     double* d_partials = nullptr;
-    double* d_sums = nullptr;   // [NACC] + scale at [NACC]
+    int64_t* d_map = nullptr;   // re-gridding table of gpe_remap_psi into this sim (allocated on first use)
+    double* d_sums = nullptr;   // [NACC] + scale at [NACC] + degenerate-norm flag at [NACC + 1]
     int64_t launches = 0;
     bool counted = false;   // registered in grid->n_sims
     // stage timing
@@ -177,12 +178,18 @@ int upload_grid(gpe_grid* g) {
     CU(e);
     e = cudaMalloc(&g->d_perm, na * sizeof(int64_t));
     if (e == cudaErrorMemoryAllocation) { cudaFree(g->d_slabs); g->d_slabs = nullptr; return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(perm)"); }
-    CU(e);
+    if (e != cudaSuccess) { cudaFree(g->d_slabs); g->d_slabs = nullptr; return cuda_fail(e, "cudaMalloc(perm)"); }
     std::vector<Slab> slabs((size_t)h.n_slabs());
     for (int64_t k = 0; k < h.n_slabs(); ++k) { slabs[k].mask = h.slab_mask[k]; slabs[k].base = h.slab_base[k]; }
-    if (!slabs.empty()) CU(cudaMemcpy(g->d_slabs, slabs.data(), slabs.size() * sizeof(Slab), cudaMemcpyHostToDevice));
-    if (h.n_active > 0)
-        CU(cudaMemcpy(g->d_perm, h.storage_to_canonical.data(), (size_t)h.n_active * sizeof(int64_t), cudaMemcpyHostToDevice));
+    e = cudaSuccess;
+    if (!slabs.empty()) e = cudaMemcpy(g->d_slabs, slabs.data(), slabs.size() * sizeof(Slab), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && h.n_active > 0)
+        e = cudaMemcpy(g->d_perm, h.storage_to_canonical.data(), (size_t)h.n_active * sizeof(int64_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {   // nothing is left allocated on a failed upload (a retry allocates again)
+        cudaFree(g->d_slabs); g->d_slabs = nullptr;
+        cudaFree(g->d_perm); g->d_perm = nullptr;
+        return cuda_fail(e, "cudaMemcpy(layout tables)");
+    }
     g->device = dev;
     g->on_device = true;
     return GPE_OK;
@@ -320,6 +327,22 @@ int rkck_step(gpe_sim* s, double t, double dt, void* stream) {
     return stage_lc(s, t + c[5] * dt, sub[5] * dt, Y[5], 5, Y, bstar, bstar[5], Y[0], stream);
 }
 
+// End of an imaginary-time run: apply the lazy scale, reset it, and report a degenerate particle number (the
+// finalise kernel kept scale 1 and raised the flag: the state is returned as it is).  Synchronises the stream.
+int flush_scale(gpe_sim* s, void* stream) {
+    KL(launch_scale(pair_dtype(s->dtype), s->buf[0], pair_count(s->dtype, s->n), s->d_sums + NACC, stream));
+    KL(launch_set_scalar(s->d_sums + NACC, 1.0, stream));
+    s->launches += 2;
+    double flag = 0.0;
+    CU(cudaMemcpyAsync(&flag, s->d_sums + NACC + 1, sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    if (flag != 0.0) {
+        CU(cudaMemsetAsync(s->d_sums + NACC + 1, 0, sizeof(double), (cudaStream_t)stream));
+        return fail(GPE_ERR_STATE, "the particle number became zero or non-finite during the imaginary-time run (no renormalisation applied)");
+    }
+    return GPE_OK;
+}
+
 int sums_to_host(gpe_sim* s, double out[NACC], void* stream) {
     CU(cudaMemcpyAsync(out, s->d_sums, NACC * sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CU(cudaStreamSynchronize((cudaStream_t)stream));
@@ -448,6 +471,19 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     if (state_bytes < 5 * bb) return fail(GPE_ERR_INVALID_ARG, "state_bytes too small (see gpe_sim_state_bytes)");
     int rc = upload_grid(g);
     if (rc) return rc;
+    {
+        // the grid's tables live on the device that was current when its first sim was created: every sim on the
+        // grid, and its state buffer, must be on that device
+        int dev = -1;
+        CU(cudaGetDevice(&dev));
+        if (dev != g->device) return fail(GPE_ERR_STATE, "the current device is not the one the grid's tables were uploaded to");
+        cudaPointerAttributes attr;
+        cudaError_t pe = cudaPointerGetAttributes(&attr, dev_state);
+        if (pe != cudaSuccess || attr.type != cudaMemoryTypeDevice || attr.device != g->device) {
+            cudaGetLastError();
+            return fail(GPE_ERR_INVALID_ARG, "dev_state is not device memory of the grid's device");
+        }
+    }
     gpe_sim* s = new (std::nothrow) gpe_sim();
     if (!s) return fail(GPE_ERR_OUT_OF_MEMORY, "host allocation");
     s->grid = g;
@@ -463,13 +499,13 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     s->kz = s->n < 300000 ? 4 : s->n < 3000000 ? 8 : s->n < 20000000 ? 16 : 32;
     for (int k = 0; k < 4; ++k) s->buf[k] = (char*)dev_state + k * bb;
     s->staging = (char*)dev_state + 4 * bb;
-    cudaError_t e = cudaMalloc(&s->d_sums, (NACC + 1) * sizeof(double));
+    cudaError_t e = cudaMalloc(&s->d_sums, (NACC + 2) * sizeof(double));
     if (e != cudaSuccess) { delete s; return e == cudaErrorMemoryAllocation ? fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc") : cuda_fail(e, "cudaMalloc"); }
     rc = build_work(s);
     if (rc) { gpe_sim_destroy(s); return rc; }
     cudaStream_t st = (cudaStream_t)stream;
     e = cudaMemsetAsync(dev_state, 0, 5 * bb, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_sums, 0, (NACC + 1) * sizeof(double), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->d_sums, 0, (NACC + 2) * sizeof(double), st);
     if (e == cudaSuccess) e = (cudaError_t)launch_set_scalar(s->d_sums + NACC, 1.0, stream);
     if (e != cudaSuccess) { gpe_sim_destroy(s); return cuda_fail(e, "state initialisation"); }
     g->n_sims += 1;
@@ -484,6 +520,7 @@ int gpe_sim_destroy(gpe_sim* s) {
     if (s->d_work) cudaFree(s->d_work);
     if (s->d_partials) cudaFree(s->d_partials);
     if (s->d_sums) cudaFree(s->d_sums);
+    if (s->d_map) cudaFree(s->d_map);
     for (int k = 0; k < 2; ++k)
         if (s->extra[k]) cudaFree(s->extra[k]);
     for (int k = 0; k < 4; ++k)
@@ -524,20 +561,17 @@ int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream) {
         while (j < ia.size() && ia[j] < ib[i]) ++j;
         map[i] = (j < ia.size() && ia[j] == ib[i]) ? (int64_t)j : -1;
     }
-    int64_t* d_map = nullptr;
-    cudaError_t e = cudaMalloc(&d_map, map.size() * sizeof(int64_t));
-    if (e == cudaErrorMemoryAllocation) return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(remap table)");
-    CU(e);
+    if (!dst->d_map) {   // kept for the life of the destination sim: a ramp re-grids after every stage
+        cudaError_t em = cudaMalloc(&dst->d_map, map.size() * sizeof(int64_t));
+        if (em == cudaErrorMemoryAllocation) return fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc(remap table)");
+        CU(em);
+    }
     cudaStream_t st = (cudaStream_t)stream;
-    e = cudaMemcpyAsync(d_map, map.data(), map.size() * sizeof(int64_t), cudaMemcpyHostToDevice, st);
-    int rc = 0;
-    if (e == cudaSuccess && src->n > 0) rc = launch_unpack(copy_dtype(src->dtype), src->buf[0], src->staging, src->grid->d_perm, src->n, stream);
-    if (e == cudaSuccess && !rc) rc = launch_remap(copy_dtype(dst->dtype), src->staging, dst->staging, d_map, dst->n, stream);
-    if (e == cudaSuccess && !rc) rc = launch_pack(copy_dtype(dst->dtype), dst->staging, dst->buf[0], dst->grid->d_perm, dst->n, stream);
-    if (e == cudaSuccess && !rc) e = cudaStreamSynchronize(st);   // the table is freed below
-    cudaFree(d_map);
-    if (e != cudaSuccess) return cuda_fail(e, "gpe_remap_psi");
-    if (rc) return cuda_fail((cudaError_t)rc, "gpe_remap_psi kernels");
+    // pageable source: the call returns once the host vector has been staged, the device copy is stream-ordered
+    CU(cudaMemcpyAsync(dst->d_map, map.data(), map.size() * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    if (src->n > 0) KL(launch_unpack(copy_dtype(src->dtype), src->buf[0], src->staging, src->grid->d_perm, src->n, stream));
+    KL(launch_remap(copy_dtype(dst->dtype), src->staging, dst->staging, dst->d_map, dst->n, stream));
+    KL(launch_pack(copy_dtype(dst->dtype), dst->staging, dst->buf[0], dst->grid->d_perm, dst->n, stream));
     src->launches += src->n > 0 ? 1 : 0;
     dst->launches += 2;
     return GPE_OK;
@@ -660,10 +694,7 @@ int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
         std::swap(s->buf[0], s->buf[1]);
     }
     // flush the lazy scale so that every other call sees a normalised state
-    KL(launch_scale(pair_dtype(s->dtype), s->buf[0], pair_count(s->dtype, s->n), s->d_sums + NACC, stream));
-    KL(launch_set_scalar(s->d_sums + NACC, 1.0, stream));
-    s->launches += 2;
-    return GPE_OK;
+    return flush_scale(s, stream);
 }
 
 int gpe_imag_step(gpe_sim* s, double dt, void* stream) { return gpe_run_imag(s, dt, 1, stream); }
@@ -684,10 +715,7 @@ int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
         s->launches += 1;
         std::swap(s->buf[0], s->buf[1]);
     }
-    KL(launch_scale(pair_dtype(s->dtype), s->buf[0], pair_count(s->dtype, s->n), s->d_sums + NACC, stream));
-    KL(launch_set_scalar(s->d_sums + NACC, 1.0, stream));
-    s->launches += 2;
-    return GPE_OK;
+    return flush_scale(s, stream);
 }
 
 int gpe_imag_split_step(gpe_sim* s, double dt, void* stream) { return gpe_run_imag_split(s, dt, 1, stream); }

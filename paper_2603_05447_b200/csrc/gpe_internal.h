@@ -154,7 +154,8 @@ int launch_remap(int dtype, const void* src_canonical, void* dst_canonical, cons
 int norm_blocks(int64_t n);
 int launch_norm_partials(int dtype, const void* storage, int64_t n, double* partials, void* stream);
 // out[k] = sum_b partials[b*NACC + k] in a fixed order (k < NACC); if scale_out != null also writes
-// scale_out[0] = sqrt(n_target / (h3 * out[0]))
+// scale_out[0] = sqrt(n_target / (h3 * out[0])), or 1 and the sticky flag scale_out[1] = 1 when out[0] is zero or
+// not finite
 int launch_finalize(const double* partials, int64_t nblk, double* out, double* scale_out,
                     double n_target, double h3, void* stream);
 int launch_scale(int dtype, void* storage, int64_t n, const double* scale, void* stream);

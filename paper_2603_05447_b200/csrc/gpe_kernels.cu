@@ -86,7 +86,13 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const double* __r
         double s = 0.0;
         for (int wv = 0; wv < FIN_THREADS / 32; ++wv) s += red[wv][threadIdx.x];
         out[threadIdx.x] = s;
-        if (threadIdx.x == 0 && scale_out) scale_out[0] = sqrt(n_target / (h3 * s));
+        if (threadIdx.x == 0 && scale_out) {
+            // a zero or non-finite particle number has no renormalisation: keep the values as they are (scale 1)
+            // and raise the sticky flag next to the scale; the host turns it into GPE_ERR_STATE at the flush
+            const bool ok = s > 0.0 && isfinite(s);
+            scale_out[0] = ok ? sqrt(n_target / (h3 * s)) : 1.0;
+            if (!ok) scale_out[1] = 1.0;
+        }
     }
 }
 

@@ -192,6 +192,10 @@ stage_kernel(const __grid_constant__ StageParams p) {
     constexpr unsigned ROW_BYTES = (unsigned)G::PY * ES;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
+    // Programmatic dependent launch: the next stage kernel of the stream may be scheduled as soon as every block of
+    // this one has started (i.e. into the slots this kernel's tail leaves idle); it stages its tables, which no
+    // kernel writes, and waits below (griddepcontrol.wait) for this kernel to complete before it touches psi.
+    asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int half = lane / LPS, t = lane % LPS;
     const int g = t >> 3, ly = t & 7;                      // row group and column of the PRx1 patch
@@ -284,6 +288,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
             qxy[e] = fma(p.hax, x * x, qy);
         }
     }
+    // everything above read the work record and the slab tables only; psi, the aux operand and the lazy scale are
+    // written by the kernels before this one
+    asm volatile("griddepcontrol.wait;\n" ::: "memory");
     double sc = 1.0, gsc = p.g;
     if (MODE == MODE_IMAG || MODE == MODE_PREP) { sc = *p.scale_in; gsc = p.g * (sc * sc); }
 
@@ -630,8 +637,17 @@ template <typename T, int R, int MODE, bool HOC, bool REAL>
 cudaError_t launch_one(const StageParams& p, cudaStream_t st) {
     constexpr int spb = STAGE_WARPS * rows_per_lane<T>() / 2;   // streams per block
     const int nblk = (p.n_work + spb - 1) / spb;
-    stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC, REAL><<<nblk, STAGE_THREADS, stage_smem<T, R, MODE, HOC, REAL>(), st>>>(p);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)nblk);
+    cfg.blockDim = dim3(STAGE_THREADS);
+    cfg.dynamicSmemBytes = stage_smem<T, R, MODE, HOC, REAL>();
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC, REAL>, p);
 }
 
 template <typename T, int R, bool HOC>

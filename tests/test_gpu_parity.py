@@ -446,3 +446,77 @@ def test_degenerate_boxes(P, dims, stencil):
     sim.set_psi_host(psi)
     sim.run_rk4(1e-3, 2)
     assert rel_max(sim.get_psi_host(), O.run_rk4(og, pot, w.g, 0.0, 1e-3, 2, psi, stencil)) < 1e-12
+
+
+def test_zero_state_has_no_renormalisation(P):
+    """A state with zero particle number cannot be renormalised: both imaginary-time runs report GPE_ERR_STATE at
+    their flush instead of handing back NaNs, and the sim stays usable."""
+    w = I.small_shell(24, 13)
+    box, pot, act, grid, sim = _make(P, w)
+    zero = np.zeros(act.size, np.complex128)
+    for run in (sim.run_imag, sim.run_imag_split):
+        sim.set_psi_host(zero)
+        with pytest.raises(P.GpeError) as e:
+            run(1e-3, 3)
+        assert e.value.code == -5
+        assert np.all(sim.get_psi_host() == 0)             # scale 1 was applied: no NaN
+    psi = I.make_psi0(w, act)
+    sim.set_psi_host(psi)
+    sim.run_imag(1e-3, 2)
+    og = O.SparseGrid(box, act, 2)
+    assert rel_max(sim.get_psi_host(), O.run_imag(og, pot, w.g, 0.0, 1e-3, 2, psi, 13)) < 1e-12
+
+
+def test_staged_ramp_with_regridding(P):
+    """The ramp as the paper runs it (PAPER.md:151-153): stage after stage of a linearly interpolated potential;
+    at the end of each stage the grid post-selection is repeated with the threshold 5 max(mu_i, mu_i+1) and the
+    wavefunction is remapped from the old grid to the new one.  Here: the 128^3, h = 0.8 replica of BASELINE
+    configs[2] (Omega = 20, g = 2000, 7-point), Delta: 0 -> 800 in 8 stages of 100 RK4 steps (dt = 2e-3, stage
+    length 0.2); mu_i is the chemical potential of the evolving state at the stage boundary (gpe_energy).  The
+    oracle does the same with energy()['mu'], active_indices and remap_psi: every grid must be identical and the
+    final state agree at the 1000-step bound."""
+    n_stage, steps, dt = 8, 100, 2e-3
+    T = steps * dt
+    base = I.config3(True).with_(nx=128, ny=128, nz=128, h=0.8, dt=dt, name="cfg3_staged_128")
+    dd = (base.delta1 - base.delta0) / n_stage
+
+    def stage_workload(s, v_cut):
+        return base.with_(delta0=base.delta0 + s * dd, delta1=base.delta0 + (s + 1) * dd, t_ramp=T, v_cut=v_cut,
+                          mask_mode=I.MASK_UNION)
+
+    # stage 0 on BASELINE's own cut; reference state on the oracle side
+    w = stage_workload(0, base.v_cut)
+    box, pot, act, grid, sim = _make(P, w)
+    psi = I.make_psi0(w, act)
+    sim.set_psi_host(psi)
+    ref = psi.copy()
+    co = CO.COracle(box, pot, act, w.stencil)
+    mu_gpu, mu_ref = sim.energy()["mu"], co.energy(w.g, 0.0, ref)["mu"]
+    sizes = [act.size]
+    keep = []                                               # sims of earlier stages stay alive until the end
+    for s in range(n_stage):
+        sim.time = 0.0
+        sim.run_rk4(dt, steps)
+        ref = co.run_rk4(w.g, 0.0, dt, steps, ref)
+        assert rel_max(sim.get_psi_host(), ref) < 1e-9, s
+        e_gpu, e_ref = sim.energy(), co.energy(w.g, T, ref)        # mu at the stage boundary, V at Delta_{s+1}
+        assert abs(e_gpu["mu"] - e_ref["mu"]) < 1e-10 * abs(e_ref["mu"])
+        if s == n_stage - 1:
+            break
+        cut_gpu, cut_ref = 5.0 * max(mu_gpu, e_gpu["mu"]), 5.0 * max(mu_ref, e_ref["mu"])
+        mu_gpu, mu_ref = e_gpu["mu"], e_ref["mu"]
+        # re-select: library on its own threshold, oracle on its own
+        w_new = stage_workload(s + 1, cut_gpu)
+        grid_new = P.Grid.from_workload(w_new)
+        box_n, pot_n, act_n = oracle_objs(stage_workload(s + 1, cut_ref))
+        assert np.array_equal(grid_new.active_indices(), act_n), s
+        sim_new = P.Sim(grid_new, w_new.dtype, w_new.stencil, w_new.g)
+        sim_new.remap_from(sim)
+        ref = O.remap_psi(act, ref, act_n)
+        assert np.array_equal(sim_new.get_psi_host() != 0, ref != 0)
+        keep.append((sim, grid))
+        sim, grid, w, act, pot = sim_new, grid_new, w_new, act_n, pot_n
+        co = CO.COracle(box_n, pot_n, act_n, w.stencil)
+        sizes.append(act_n.size)
+    assert len(set(sizes)) > 1                              # the mask really followed the cloud
+    assert abs(sim.norm() - co.norm(ref)) < 1e-10

@@ -351,8 +351,10 @@ def test_P12_counts_fixture_config1_config2():
         assert act.size == counts[w.name]["n_active"]
         assert st.size == counts[w.name]["n_stored"]
     # the survey's independent count script gave the same numbers
-    assert counts["cfg1_harmonic_48"] == {"n_active": 67080, "n_stored": 67080 + 9888}
-    assert counts["cfg2_bubble_256"] == {"n_active": 1215760, "n_stored": 1215760 + 418000}
+    sv = {"cfg1_harmonic_48": (67080, 9888), "cfg2_bubble_256": (1215760, 418000), "cfg3a_ramp_union_512": (38495288, 922496),
+          "cfg3b_ramp_final_512": (9730864, 1671856), "cfg4_ellipsoid_1024_c128": (31523416, 5942744)}   # SURVEY.md:237-241
+    for name, (na, halo) in sv.items():
+        assert (counts[name]["n_active"], counts[name]["n_stored"]) == (na, na + halo), name
 
 
 def test_P12_mask_is_ball_for_harmonic():

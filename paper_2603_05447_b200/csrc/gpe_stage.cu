@@ -133,6 +133,7 @@ constexpr int KZMAX = 32;                 // planes per stream (host splits work
 __host__ __device__ constexpr int pf_of(int radius) { return radius == 1 ? GPE_PF_R1 : 3; }
 constexpr int STAGE_WARPS = STAGE_THREADS / 32;
 
+
 // Shared memory of one stream.  Plane slot: (8+2R) rows (x) of PY values, the tile at rows/cols R..R+7 and
 // the star halo around it.
 template <typename T, int R, bool AUX, bool HOC = false, bool REAL = false> struct Geo {

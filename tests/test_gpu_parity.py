@@ -471,13 +471,13 @@ def test_staged_ramp_with_regridding(P):
     """The ramp as the paper runs it (PAPER.md:151-153): stage after stage of a linearly interpolated potential;
     at the end of each stage the grid post-selection is repeated with the threshold 5 max(mu_i, mu_i+1) and the
     wavefunction is remapped from the old grid to the new one.  Here: the 128^3, h = 0.8 replica of BASELINE
-    configs[2] (Omega = 20, g = 2000, 7-point), Delta: 0 -> 800 in 8 stages of 100 RK4 steps (dt = 2e-3, stage
-    length 0.2); mu_i is the chemical potential of the evolving state at the stage boundary (gpe_energy).  The
+    configs[2] (Omega = 20, g = 2000, 7-point), Delta: 0 -> 80 in 8 stages of 100 RK4 steps (dt = 2e-3, stage
+    length 0.2; the full 0 -> 800 in this time is far from adiabatic and leaves RK4's stability range); mu_i is the chemical potential of the evolving state at the stage boundary (gpe_energy).  The
     oracle does the same with energy()['mu'], active_indices and remap_psi: every grid must be identical and the
     final state agree at the 1000-step bound."""
     n_stage, steps, dt = 8, 100, 2e-3
     T = steps * dt
-    base = I.config3(True).with_(nx=128, ny=128, nz=128, h=0.8, dt=dt, name="cfg3_staged_128")
+    base = I.config3(True).with_(nx=128, ny=128, nz=128, h=0.8, dt=dt, delta1=80.0, name="cfg3_staged_128")
     dd = (base.delta1 - base.delta0) / n_stage
 
     def stage_workload(s, v_cut):

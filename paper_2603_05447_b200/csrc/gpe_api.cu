@@ -144,6 +144,15 @@ int build_work(gpe_sim* s) {
             const int64_t e0 = r.eoff[0] + s0, e1 = r.eoff[0] + s1 - 1;
             r.pos0 = h.slab_base[e0];
             r.npts = (int32_t)(h.slab_base[e1] + __builtin_popcountll(h.slab_mask[e1]) - r.pos0);
+            // the R planes below the piece matter through the z direction of the own columns only (star stencils):
+            // a piece that starts a run has nothing there and skips them; the 19-/27-point stencils also see the
+            // neighbour tiles' points in those planes (xz / yz edges) and always read them
+            r.lead = s->radius;
+            if (!s->hoc) {
+                bool any = false;
+                for (int z = std::max(s0 - s->radius, (int)h.tile_zlo[k]); z < s0; ++z) any = any || h.slab_mask[r.eoff[0] + z] != 0;
+                if (!any) r.lead = 0;
+            }
             recs.push_back(r);
         }
     }

@@ -71,7 +71,8 @@ struct alignas(16) WorkRec {
     int32_t zhi[NTILE];
     long long pos0;     // storage position of the first point of the piece
     int32_t npts;       // points in the piece (contiguous in storage from pos0)
-    int32_t pad[3];
+    int32_t lead;       // overlap planes below z0 the stream reads: R, or 0 when the tile holds no point in them
+    int32_t pad[2];
 };
 static_assert(sizeof(WorkRec) == 192, "WorkRec layout");
 

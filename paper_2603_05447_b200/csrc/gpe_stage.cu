@@ -205,8 +205,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
     const WorkRec* __restrict__ w = p.work + (valid ? sidx : 0);
 
     const int z0 = w->z0, nz = valid ? w->nz : 0;
-    const int kstart = z0 - R;
-    const int ne = nz > 0 ? nz + 2 * R : 0;                // planes kstart .. kstart+ne-1 are touched
+    const int lead = w->lead;                              // overlap planes read below z0 (R, or 0: nothing there)
+    const int kstart = z0 - lead;
+    const int ne = nz > 0 ? nz + lead + R : 0;             // planes kstart .. kstart+ne-1 are touched
 
     const unsigned sb = (unsigned)__cvta_generic_to_shared(smem_raw) + (unsigned)((warp * SPW + half) * G::STREAM_BYTES);
     const unsigned ring = sb, auxring = sb + G::RING_BYTES, smask = sb + G::MASK_OFF, sbase = sb + G::BASE_OFF;
@@ -314,7 +315,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 }
             }
             // 19-point: the overlap planes need their in-plane face sums too (they are the xz / yz edge neighbours)
-            if (MODE != MODE_PREP && (HOC || (i >= R && i < ne - R))) {
+            if (MODE != MODE_PREP && (HOC || (i >= lead && i < ne - R))) {
                 const unsigned ti = (unsigned)((1 + hq) * G::NE + i);
                 const uint2 m = lds_u2(smask + ti * 8u);
                 const unsigned b = lds_u1(sbase + ti * 4u);
@@ -337,7 +338,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
             }
             if (HAS_AUX) {
                 const int ia = i - R;
-                if (ia >= R && ia < ne - R) {
+                if (ia >= lead && ia < ne - R) {
                     const uint2 m = lds_u2(smask + (unsigned)ia * 8u);
                     const unsigned word = ghi ? m.y : m.x;
                     const unsigned bc = lds_u1(sbase + (unsigned)ia * 4u) + (ghi ? (unsigned)__popc(m.x) : 0u);
@@ -384,7 +385,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
         // ---- output plane: activity bits and storage positions --------------------------------------------
         unsigned cword = 0u, cbase = 0u;
         bool cany = false;                                      // the slab of plane c holds points (stream-uniform)
-        if (ic >= R) {
+        if (ic >= lead) {
             const uint2 m = lds_u2(smask + (unsigned)ic * 8u);
             cword = ghi ? m.y : m.x;
             cbase = lds_u1(sbase + (unsigned)ic * 4u) + (ghi ? (unsigned)__popc(m.x) : 0u);
@@ -564,7 +565,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
             }
         }
         // ---- in-plane part (only planes of the stream itself are ever finished) ----------------------------------
-        if (!HOC && MODE != MODE_PREP && i >= R && i < ne - R) {
+        if (!HOC && MODE != MODE_PREP && i >= lead && i < ne - R) {
             // x direction: source rows r = -R .. PR-1+R of column ly; rows 0..PR-1 are the patch itself
 #pragma unroll
             for (int r = -R; r <= PR - 1 + R; ++r) {

@@ -43,6 +43,9 @@ struct gpe_sim {
     int32_t n_blocks = 0;
     double* d_partials = nullptr;
     int64_t* d_map = nullptr;   // re-gridding table of gpe_remap_psi into this sim (allocated on first use)
+    double* h_flag = nullptr;   // pinned copy of the degenerate-norm flag, filled asynchronously at the end of a run
+    cudaEvent_t ev_flag = nullptr;
+    bool flag_pending = false;
     double* d_sums = nullptr;   // [NACC] + scale at [NACC] + degenerate-norm flag at [NACC + 1]
     int64_t launches = 0;
     bool counted = false;   // registered in grid->n_sims
@@ -336,18 +339,34 @@ int rkck_step(gpe_sim* s, double t, double dt, void* stream) {
     return stage_lc(s, t + c[5] * dt, sub[5] * dt, Y[5], 5, Y, bstar, bstar[5], Y[0], stream);
 }
 
-// End of an imaginary-time run: apply the lazy scale, reset it, and report a degenerate particle number (the
-// finalise kernel kept scale 1 and raised the flag: the state is returned as it is).  Synchronises the stream.
+// End of an imaginary-time run: apply the lazy scale, reset it, and fetch the degenerate-norm flag (the finalise
+// kernel kept scale 1 and raised it: the state is left as it is) into pinned memory WITHOUT synchronising: a loop of
+// single steps stays asynchronous.  check_flag() reports it at the next call that can know.
 int flush_scale(gpe_sim* s, void* stream) {
     KL(launch_scale(pair_dtype(s->dtype), s->buf[0], pair_count(s->dtype, s->n), s->d_sums + NACC, stream));
     KL(launch_set_scalar(s->d_sums + NACC, 1.0, stream));
     s->launches += 2;
-    double flag = 0.0;
-    CU(cudaMemcpyAsync(&flag, s->d_sums + NACC + 1, sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
-    CU(cudaStreamSynchronize((cudaStream_t)stream));
-    if (flag != 0.0) {
+    CU(cudaMemcpyAsync(s->h_flag, s->d_sums + NACC + 1, sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CU(cudaEventRecord(s->ev_flag, (cudaStream_t)stream));
+    s->flag_pending = true;
+    return GPE_OK;
+}
+
+// synced = the caller has just synchronised the stream the run was enqueued on
+int check_flag(gpe_sim* s, bool synced, void* stream) {
+    if (!s->flag_pending) return GPE_OK;
+    if (!synced) {
+        cudaError_t q = cudaEventQuery(s->ev_flag);
+        if (q == cudaErrorNotReady) return GPE_OK;         // still running: a later call reports it
+        CU(q);
+    } else {
+        CU(cudaEventSynchronize(s->ev_flag));
+    }
+    s->flag_pending = false;
+    if (*s->h_flag != 0.0) {
+        *s->h_flag = 0.0;
         CU(cudaMemsetAsync(s->d_sums + NACC + 1, 0, sizeof(double), (cudaStream_t)stream));
-        return fail(GPE_ERR_STATE, "the particle number became zero or non-finite during the imaginary-time run (no renormalisation applied)");
+        return fail(GPE_ERR_STATE, "the particle number became zero or non-finite during an imaginary-time run (no renormalisation was applied)");
     }
     return GPE_OK;
 }
@@ -510,6 +529,9 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     s->staging = (char*)dev_state + 4 * bb;
     cudaError_t e = cudaMalloc(&s->d_sums, (NACC + 2) * sizeof(double));
     if (e != cudaSuccess) { delete s; return e == cudaErrorMemoryAllocation ? fail(GPE_ERR_OUT_OF_MEMORY, "cudaMalloc") : cuda_fail(e, "cudaMalloc"); }
+    e = cudaMallocHost(&s->h_flag, sizeof(double));
+    if (e == cudaSuccess) { *s->h_flag = 0.0; e = cudaEventCreateWithFlags(&s->ev_flag, cudaEventDisableTiming); }
+    if (e != cudaSuccess) { gpe_sim_destroy(s); return cuda_fail(e, "pinned flag / event"); }
     rc = build_work(s);
     if (rc) { gpe_sim_destroy(s); return rc; }
     cudaStream_t st = (cudaStream_t)stream;
@@ -530,6 +552,8 @@ int gpe_sim_destroy(gpe_sim* s) {
     if (s->d_partials) cudaFree(s->d_partials);
     if (s->d_sums) cudaFree(s->d_sums);
     if (s->d_map) cudaFree(s->d_map);
+    if (s->h_flag) cudaFreeHost(s->h_flag);
+    if (s->ev_flag) cudaEventDestroy(s->ev_flag);
     for (int k = 0; k < 2; ++k)
         if (s->extra[k]) cudaFree(s->extra[k]);
     for (int k = 0; k < 4; ++k)
@@ -603,7 +627,7 @@ int gpe_get_psi_host(gpe_sim* s, void* host_psi_canonical, void* stream) {
     if (rc) return rc;
     CU(cudaMemcpyAsync(host_psi_canonical, s->staging, (size_t)s->n * s->csize, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CU(cudaStreamSynchronize((cudaStream_t)stream));
-    return GPE_OK;
+    return check_flag(s, true, stream);
 }
 
 int gpe_set_time(gpe_sim* s, double t) {
@@ -694,6 +718,7 @@ int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
     if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
     if (s->n == 0 || nsteps == 0) return GPE_OK;
+    { int rcf = check_flag(s, false, stream); if (rcf) return rcf; }
     const double h3 = cell_volume(s->grid->h.box);
     for (int64_t n = 0; n < nsteps; ++n) {
         int rc = stage(s, MODE_IMAG, s->t, dt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
@@ -712,6 +737,7 @@ int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
     if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
     if (s->n == 0 || nsteps == 0) return GPE_OK;
+    { int rcf = check_flag(s, false, stream); if (rcf) return rcf; }
     const double h3 = cell_volume(s->grid->h.box);
     const double hdt = 0.5 * dt;
     for (int64_t n = 0; n < nsteps; ++n) {
@@ -738,6 +764,7 @@ int gpe_norm(gpe_sim* s, double* out_host, void* stream) {
     s->launches += 2;
     double sums[NACC];
     int rc = sums_to_host(s, sums, stream);
+    if (!rc) rc = check_flag(s, true, stream);
     if (rc) return rc;
     const double v = h3 * sums[0];
     if (!std::isfinite(v)) return fail(GPE_ERR_STATE, "norm is not finite");
@@ -755,6 +782,7 @@ int gpe_energy(gpe_sim* s, gpe_energy_out* o, void* stream) {
     s->launches += 1;
     double sums[NACC];
     rc = sums_to_host(s, sums, stream);
+    if (!rc) rc = check_flag(s, true, stream);
     if (rc) return rc;
     gpe_energy_out r;
     r.kin = h3 * sums[0];

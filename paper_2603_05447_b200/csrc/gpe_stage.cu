@@ -171,6 +171,16 @@ template <> struct KW<float> {
 // imaginary part of a value: identically zero for a real-valued state (REAL), where it is not computed at all
 #define YV(expr) (REAL ? (T)0 : (T)(expr))
 
+// acc += w * v for a real weight and a complex value: complex64 uses Blackwell's packed FP32 FMA (FFMA2: both
+// components in one instruction, same rounding as two FFMAs)
+template <bool REAL> __device__ __forceinline__ void caxpy(double2& acc, double w, const double2& v) {
+    acc.x = fma(w, v.x, acc.x);
+    if (!REAL) acc.y = fma(w, v.y, acc.y);
+}
+template <bool REAL> __device__ __forceinline__ void caxpy(float2& acc, float w, const float2& v) {
+    acc = __ffma2_rn(make_float2(w, w), v, acc);
+}
+
 __host__ __device__ constexpr bool mode_has_aux(int mode) { return mode == MODE_S2 || mode == MODE_S3 || mode == MODE_S4; }
 
 template <typename T, int R, int MODE, int PR, bool HOC, bool REAL>
@@ -415,6 +425,26 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 }
             }
         }
+        // ---- MODE_LC: warm the L2 with the earlier stage states of the plane finished two steps from now (the
+        //      loads above are consumed within their own step: from DRAM they would stall it) -------------------
+        if (MODE == MODE_LC && !REAL) {
+            const int ip = ic + 2;
+            if (ip >= lead && ip < ne - R) {
+                const uint2 m = lds_u2(smask + (unsigned)ip * 8u);
+                const unsigned wd = ghi ? m.y : m.x;
+                const unsigned bs = lds_u1(sbase + (unsigned)ip * 4u) + (ghi ? (unsigned)__popc(m.x) : 0u);
+#pragma unroll
+                for (int j = 0; j < MAX_LC_AUX; ++j) {
+                    if (j < p.n_aux) {
+                        const C* aj = reinterpret_cast<const C*>(p.auxn[j]);
+#pragma unroll
+                        for (int e = 0; e < PR; ++e)
+                            if ((wd >> (rb0 + 8 * e)) & 1u)
+                                asm volatile("prefetch.global.L2 [%0];\n" ::"l"(aj + (bs + (unsigned)__popc(wd & bm[e]))));
+                    }
+                }
+            }
+        }
         // ---- psi(k) of the patch ------------------------------------------------------------------------
         C v[PR];
 #pragma unroll
@@ -456,11 +486,9 @@ stage_kernel(const __grid_constant__ StageParams p) {
         // ---- psi(k) completes the z part of planes k-1 .. k-R -------------------------------------------
 #pragma unroll
         for (int e = 0; e < PR; ++e) {
-            AO[e].x = fma(KW<T>::w(p, 2, R), v[e].x, AO[e].x);
-            AO[e].y = YV(fma(KW<T>::w(p, 2, R), v[e].y, AO[e].y));
+            caxpy<REAL>(AO[e], KW<T>::w(p, 2, R), v[e]);
             if (R == 2) {
-                AN[e].x = fma(KW<T>::w(p, 2, 1), v[e].x, AN[e].x);
-                AN[e].y = YV(fma(KW<T>::w(p, 2, 1), v[e].y, AN[e].y));
+                caxpy<REAL>(AN[e], KW<T>::w(p, 2, 1), v[e]);
             }
             if (HOC && MODE != MODE_PREP) {                     // the xz / yz edge neighbours of plane k-1 in plane k
                 AO[e].x += G[e].x;
@@ -548,14 +576,13 @@ stage_kernel(const __grid_constant__ StageParams p) {
             if (R == 2) {
                 an.x = KW<T>::w(p, 2, 2) * PO[e].x;
                 an.y = YV(KW<T>::w(p, 2, 2) * PO[e].y);
-                an.x = fma(KW<T>::w(p, 2, 1), PN[e].x, an.x);
-                an.y = YV(fma(KW<T>::w(p, 2, 1), PN[e].y, an.y));
+                caxpy<REAL>(an, KW<T>::w(p, 2, 1), PN[e]);
             } else {
                 an.x = KW<T>::w(p, 2, 1) * PO[e].x;
                 an.y = YV(KW<T>::w(p, 2, 1) * PO[e].y);
             }
-            AO[e].x = fma(KW<T>::c(p), v[e].x, an.x);
-            AO[e].y = YV(fma(KW<T>::c(p), v[e].y, an.y));
+            AO[e] = an;
+            caxpy<REAL>(AO[e], KW<T>::c(p), v[e]);
             PO[e] = v[e];
             if (HOC && MODE != MODE_PREP) {
                 // faces and diagonals of plane k, and plane k-1's share of the xz / yz edges
@@ -574,8 +601,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
                 for (int a = 0; a < PR; ++a) {
                     const int d = r > a ? r - a : a - r;
                     if (d >= 1 && d <= R) {
-                        AO[a].x = fma(KW<T>::w(p, 0, d), val.x, AO[a].x);
-                        AO[a].y = YV(fma(KW<T>::w(p, 0, d), val.y, AO[a].y));
+                        caxpy<REAL>(AO[a], KW<T>::w(p, 0, d), val);
                     }
                 }
             }
@@ -587,8 +613,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     if (cc == 0) continue;
                     const C val = lds_c(so + (unsigned)(a * (int)ROW_BYTES + cc * (int)ES), (EL*)nullptr);
                     const int d = cc > 0 ? cc : -cc;
-                    AO[a].x = fma(KW<T>::w(p, 1, d), val.x, AO[a].x);
-                    AO[a].y = YV(fma(KW<T>::w(p, 1, d), val.y, AO[a].y));
+                    caxpy<REAL>(AO[a], KW<T>::w(p, 1, d), val);
                 }
             }
         }

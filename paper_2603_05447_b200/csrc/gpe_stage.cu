@@ -33,6 +33,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <cstdlib>
 
 #include "gpe_internal.h"
 
@@ -671,7 +672,8 @@ cudaError_t launch_one(const StageParams& p, cudaStream_t st) {
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    static const int pdl = [] { const char* e = getenv("GPE_PDL"); return e ? atoi(e) : 1; }();   // GPE_PDL=0: plain launches
+    attr[0].val.programmaticStreamSerializationAllowed = pdl;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC, REAL>, p);

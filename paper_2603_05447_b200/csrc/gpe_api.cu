@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -46,6 +47,21 @@ struct gpe_sim {
     double* h_flag = nullptr;   // pinned copy of the degenerate-norm flag, filled asynchronously at the end of a run
     cudaEvent_t ev_flag = nullptr;
     bool flag_pending = false;
+    // CUDA graph of RK4_GRAPH_STEPS steps for runs on small grids in a potential that does not change during the run
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t rk4_exec = nullptr;
+    bool graph_off = false;     // capture failed once, or GPE_GRAPH=0
+    struct GraphKey {
+        double dt = 0.0, delta = 0.0, g = 0.0, w27[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        void* buf[4] = {nullptr, nullptr, nullptr, nullptr};
+        const void* work = nullptr;
+        int32_t n_blocks = 0;
+        bool custom27 = false;
+        bool operator==(const GraphKey& o) const {
+            return dt == o.dt && delta == o.delta && g == o.g && std::memcmp(w27, o.w27, sizeof(w27)) == 0 &&
+                   std::memcmp(buf, o.buf, sizeof(buf)) == 0 && work == o.work && n_blocks == o.n_blocks && custom27 == o.custom27;
+        }
+    } rk4_key;
     double* d_sums = nullptr;   // [NACC] + scale at [NACC] + degenerate-norm flag at [NACC + 1]
     int64_t launches = 0;
     bool counted = false;   // registered in grid->n_sims
@@ -160,6 +176,7 @@ int build_work(gpe_sim* s) {
         }
     }
     if (recs.size() > (size_t)0x7fffffff) return fail(GPE_ERR_UNSUPPORTED, "too many work pieces");
+    if (s->rk4_exec) { cudaGraphExecDestroy(s->rk4_exec); s->rk4_exec = nullptr; }   // captured with the old work records
     if (s->d_work) { cudaFree(s->d_work); s->d_work = nullptr; }
     if (s->d_partials) { cudaFree(s->d_partials); s->d_partials = nullptr; }
     s->n_blocks = (int32_t)recs.size();
@@ -371,6 +388,56 @@ int check_flag(gpe_sim* s, bool synced, void* stream) {
     return GPE_OK;
 }
 
+constexpr int RK4_GRAPH_STEPS = 8;
+constexpr int64_t GRAPH_MAX_POINTS = 4000000;   // above this the stage kernels are long enough for the host to keep ahead
+
+// RK4 steps [0, nfull * RK4_GRAPH_STEPS) of a run in a potential that is the same at every stage time of the run:
+// the four launches of a step have the same parameters in every step, so RK4_GRAPH_STEPS steps are captured once
+// into a CUDA graph (programmatic dependent launches included) and replayed; the host leaves the loop
+// (PAPER.md:87 keeps the iteration on the device for the same reason).  Returns the number of steps done (0 = the
+// caller runs everything step by step); results are bit-identical to the step-by-step path (same kernels, same
+// parameters, same order).
+int64_t rk4_graph_steps(gpe_sim* s, double t0, double dt, int64_t nsteps, void* stream) {
+    static const bool env_off = [] { const char* e = getenv("GPE_GRAPH"); return e && atoi(e) == 0; }();
+    if (env_off || s->graph_off || s->timing || s->n_blocks <= 0 || s->n > GRAPH_MAX_POINTS || nsteps < 2 * RK4_GRAPH_STEPS) return 0;
+    const gpe_potential& pot = s->grid->h.pot;
+    const double d0 = delta_of_t(pot, t0), d1 = delta_of_t(pot, t0 + (double)nsteps * dt);
+    if (pot.kind == GPE_POT_DRESSED && d0 != d1) return 0;   // Delta(t) is monotone: equal ends = constant in between
+    gpe_sim::GraphKey key;
+    key.dt = dt; key.delta = pot.kind == GPE_POT_DRESSED ? d0 : 0.0; key.g = s->g;
+    std::memcpy(key.w27, s->w27, sizeof(key.w27));
+    for (int k = 0; k < 4; ++k) key.buf[k] = s->buf[k];
+    key.work = s->d_work; key.n_blocks = s->n_blocks; key.custom27 = s->custom27;
+    if (!s->rk4_exec || !(key == s->rk4_key)) {
+        if (s->rk4_exec) { cudaGraphExecDestroy(s->rk4_exec); s->rk4_exec = nullptr; }
+        if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+            cudaGetLastError(); s->graph_off = true; return 0;
+        }
+        const int64_t launches0 = s->launches;
+        cudaGraph_t graph = nullptr;
+        bool ok = cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+        for (int k = 0; ok && k < RK4_GRAPH_STEPS; ++k) ok = rk4_step(s, t0, dt, s->cap_stream) == GPE_OK;
+        cudaError_t ee = cudaStreamEndCapture(s->cap_stream, &graph);
+        ok = ok && ee == cudaSuccess && graph != nullptr;
+        if (ok) ok = cudaGraphInstantiate(&s->rk4_exec, graph, 0) == cudaSuccess;
+        if (graph) cudaGraphDestroy(graph);
+        s->launches = launches0;                            // nothing ran during the capture
+        if (!ok) { cudaGetLastError(); s->rk4_exec = nullptr; s->graph_off = true; return 0; }
+        s->rk4_key = key;
+    }
+    const int64_t nfull = nsteps / RK4_GRAPH_STEPS;
+    for (int64_t k = 0; k < nfull; ++k) {
+        if (cudaGraphLaunch(s->rk4_exec, (cudaStream_t)stream) != cudaSuccess) {
+            cudaGetLastError();
+            s->graph_off = true;
+            s->launches += k * RK4_GRAPH_STEPS * 4;
+            return k * RK4_GRAPH_STEPS;
+        }
+    }
+    s->launches += nfull * RK4_GRAPH_STEPS * 4;
+    return nfull * RK4_GRAPH_STEPS;
+}
+
 int sums_to_host(gpe_sim* s, double out[NACC], void* stream) {
     CU(cudaMemcpyAsync(out, s->d_sums, NACC * sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CU(cudaStreamSynchronize((cudaStream_t)stream));
@@ -554,6 +621,8 @@ int gpe_sim_destroy(gpe_sim* s) {
     if (s->d_map) cudaFree(s->d_map);
     if (s->h_flag) cudaFreeHost(s->h_flag);
     if (s->ev_flag) cudaEventDestroy(s->ev_flag);
+    if (s->rk4_exec) cudaGraphExecDestroy(s->rk4_exec);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     for (int k = 0; k < 2; ++k)
         if (s->extra[k]) cudaFree(s->extra[k]);
     for (int k = 0; k < 4; ++k)
@@ -665,7 +734,7 @@ int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     if (s->dtype == GPE_R64) return fail(GPE_ERR_UNSUPPORTED, "real-time evolution needs a complex state (GPE_C64 / GPE_C128)");
     if (!std::isfinite(dt) || nsteps < 0) return fail(GPE_ERR_INVALID_ARG, "bad dt or nsteps");
     const double t0 = s->t;
-    for (int64_t n = 0; n < nsteps; ++n) {
+    for (int64_t n = rk4_graph_steps(s, t0, dt, nsteps, stream); n < nsteps; ++n) {
         int rc = rk4_step(s, t0 + (double)n * dt, dt, stream);
         if (rc) return rc;
     }

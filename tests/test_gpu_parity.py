@@ -522,3 +522,38 @@ def test_staged_ramp_with_regridding(P):
         sizes.append(act_n.size)
     assert len(set(sizes)) > 1                              # the mask really followed the cloud
     assert abs(sim.norm() - co.norm(ref)) < 1e-10
+
+
+@pytest.mark.parametrize("dtype", ["complex128", "complex64"])
+def test_graph_replay_is_bit_identical(P, dtype):
+    """Runs of 16 or more steps on small grids in a static potential replay a captured CUDA graph of 8 steps
+    (gpe_run_rk4): same kernels, same parameters, same order, so the state is bit-identical to the one reached step
+    by step; a ramped potential (parameters change every stage) takes the step-by-step path and agrees with it too."""
+    w = I.config1().with_(dtype=dtype)
+    box, pot, act, grid, sim = _make(P, w)
+    psi = I.make_psi0(w, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    sim.run_rk4(w.dt, 43)                                   # 5 graph replays + 3 single steps
+    got = sim.get_psi_host().copy()
+    assert abs(sim.time - 43 * w.dt) < 1e-15
+    sim.set_psi_host(psi)
+    sim.time = 0.0
+    for _ in range(43):
+        sim.run_rk4(w.dt, 1)
+    assert np.array_equal(sim.get_psi_host(), got)
+    co = CO.COracle(box, pot, act, w.stencil)
+    assert rel_max(got, co.run_rk4(w.g, 0.0, w.dt, 43, psi.astype(np.complex128))) < (1e-11 if dtype == "complex128" else 1e-4)
+    # second run on the same sim reuses the graph; a changed dt rebuilds it
+    sim.run_rk4(w.dt, 16)
+    sim.run_rk4(0.5 * w.dt, 16)
+    ref = co.run_rk4(w.g, 43 * w.dt, w.dt, 16, got.astype(np.complex128))
+    ref = co.run_rk4(w.g, 59 * w.dt, 0.5 * w.dt, 16, ref)
+    assert rel_max(sim.get_psi_host(), ref) < (1e-11 if dtype == "complex128" else 1e-4)
+    # ramped dressed potential: no graph, still right
+    wr = I.small_shell(24, 13, dtype).with_(delta0=14.0, delta1=22.0, t_ramp=0.05)
+    box, pot, act, grid, sim = _make(P, wr)
+    psi = I.make_psi0(wr, act).astype(sim.npdtype)
+    sim.set_psi_host(psi)
+    sim.run_rk4(wr.dt, 20)
+    og = O.SparseGrid(box, act, 2)
+    assert rel_max(sim.get_psi_host(), O.run_rk4(og, pot, wr.g, 0.0, wr.dt, 20, psi.astype(np.complex128), 13)) < (1e-11 if dtype == "complex128" else 1e-4)

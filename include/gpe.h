@@ -183,7 +183,10 @@ int gpe_apply_H(gpe_sim* s, double t, const void* dev_in_canonical, void* dev_ou
 /* a4: one / nsteps classic RK4 steps of i dpsi/dt = H psi (PAPER.md:71 Eq. 8, :91 Eq. 9) as four fused
  * stage kernels in the stage-state form (Eq. A6-A7, A10-A11).  V is evaluated at the stage times
  * t, t+dt/2, t+dt/2, t+dt.  Step n of a run starts at t_start + n*dt (a product, not a running sum); the
- * sim clock ends at t_start + nsteps*dt. */
+ * sim clock ends at t_start + nsteps*dt.  Asynchronous on `stream`.  Runs of 16 or more steps on grids below 4e6
+ * points whose potential does not change during the run are replayed from a CUDA graph of 8 steps that the library
+ * captures on a stream of its own (same kernels, parameters and order: bit-identical results; the environment
+ * variable GPE_GRAPH=0 turns it off, GPE_PDL=0 turns off programmatic dependent launch of the stage kernels). */
 int gpe_step_rk4(gpe_sim* s, double dt, void* stream);
 int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 

@@ -231,9 +231,12 @@ int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream);
  *                                                        forward Euler method"
  *   psi <- psi exp(-V dt/2) (1 - g |psi|^2 dt/2)        Eq. 7 once more
  *   psi <- psi sqrt(n_target / (h^3 sum |psi|^2))        renormalisation
- * Three stage launches per iteration (pointwise Eq. 7 with the lazily applied scale of the previous iteration;
- * Euler half step; Euler half step + Eq. 7 + block partial sums) and a one-block finalise; exp(-V dt/2) is
- * evaluated analytically per point (no propagator array is read).  The scale is flushed at the end of the call.
+ * Two stencil launches per iteration, as the paper's K1 / K2 (:87): K1 applies Eq. 7 and the lazily applied scale of
+ * the previous iteration to every value while it is staged for the stencil (own and halo) and takes the first Euler
+ * half step; K2 takes the second Euler half step, applies Eq. 7 and writes block partial sums; then a one-block
+ * finalise.  exp(-V dt/2) is evaluated analytically per value (no propagator array is read).  GPE_K1=0 in the
+ * environment (read per call) runs the bit-identical three-launch form (pointwise Eq. 7, Euler half step, Euler half
+ * step + Eq. 7).  The scale is flushed at the end of the call.
  * With a GPE_R64 sim the state is real (:67).  Same arguments and errors as gpe_run_imag. */
 int gpe_imag_split_step(gpe_sim* s, double dt, void* stream);
 int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream);

@@ -809,15 +809,25 @@ int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     { int rcf = check_flag(s, false, stream); if (rcf) return rcf; }
     const double h3 = cell_volume(s->grid->h.box);
     const double hdt = 0.5 * dt;
+    const char* k1env = getenv("GPE_K1");                   // GPE_K1=0: three launches (PREP, KIN, SPLITB); read per call
+    const bool k1 = k1env ? atoi(k1env) != 0 : true;
     for (int64_t n = 0; n < nsteps; ++n) {
         // A holds the un-normalised state of the previous iteration; its scale sits in d_sums[NACC]
-        int rc = stage(s, MODE_PREP, s->t, hdt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
-        if (!rc) rc = stage(s, MODE_KIN, s->t, hdt, s->buf[1], nullptr, s->buf[0], nullptr, stream);
-        if (!rc) rc = stage(s, MODE_SPLITB, s->t, hdt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
+        int rc;
+        if (k1) {
+            // the paper's two stencil kernels: K1 = Eq. 7 half step + lazy scale applied while loading, first
+            // Euler half step; K2 = second Euler half step + Eq. 7 + partial sums.  4 values per point and iteration.
+            rc = stage(s, MODE_KINP, s->t, hdt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
+            if (!rc) rc = stage(s, MODE_SPLITB, s->t, hdt, s->buf[1], nullptr, s->buf[0], nullptr, stream);
+        } else {
+            rc = stage(s, MODE_PREP, s->t, hdt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
+            if (!rc) rc = stage(s, MODE_KIN, s->t, hdt, s->buf[1], nullptr, s->buf[0], nullptr, stream);
+            if (!rc) rc = stage(s, MODE_SPLITB, s->t, hdt, s->buf[0], nullptr, s->buf[1], nullptr, stream);
+        }
         if (rc) return rc;
         KL(launch_finalize(s->d_partials, s->n_blocks, s->d_sums, s->d_sums + NACC, s->n_target, h3, stream));
         s->launches += 1;
-        std::swap(s->buf[0], s->buf[1]);
+        if (!k1) std::swap(s->buf[0], s->buf[1]);
     }
     return flush_scale(s, stream);
 }

@@ -99,7 +99,10 @@ enum Mode : int {
     MODE_KIN = 8,    // out1 = c - ca T c                                                          (first Euler half step)
     MODE_SPLITB = 9, // u = c - ca T c; out1 = u exp(-V ca) (1 - g ca |u|^2); partial sum of |out1|^2
     // general stage of the memory-optimised Runge-Kutta form (PAPER.md:276-281 Eq. A6-A7; used for RKCK, A12-A13):
-    MODE_LC = 10     // out1 = sum_{j < n_aux} coef[j] auxn[j] + coefc c + ca * f(c)
+    MODE_LC = 10,    // out1 = sum_{j < n_aux} coef[j] auxn[j] + coefc c + ca * f(c)
+    // the paper's kernel K1: MODE_PREP folded into MODE_KIN's load -- every value staged for the stencil
+    // (own and halo) becomes a = s c exp(-V ca) (1 - g ca |s c|^2) in shared memory, then out1 = a - ca T a
+    MODE_KINP = 11
 };
 constexpr int MAX_LC_AUX = 5;
 constexpr int NACC = 4;           // accumulators per block in the partial-sum array

@@ -92,6 +92,15 @@ __device__ __forceinline__ double2 lds_c(unsigned addr, Re8*) {
     v.y = 0.0;
     return v;
 }
+__device__ __forceinline__ void sts_c(unsigned addr, double2 v, double2*) {
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};\n" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void sts_c(unsigned addr, float2 v, float2*) {
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};\n" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void sts_c(unsigned addr, double2 v, Re8*) {
+    asm volatile("st.shared.f64 [%0], %1;\n" ::"r"(addr), "d"(v.x) : "memory");
+}
 __device__ __forceinline__ uint2 lds_u2(unsigned addr) {
     uint2 v;
     asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];\n" : "=r"(v.x), "=r"(v.y) : "r"(addr));
@@ -123,6 +132,25 @@ __device__ __forceinline__ double fast_sqrt(double s) {
     r = fma(-g, g, s);          // residual s - g^2
     g = fma(r, h, g);
     return s > 0.0 ? g : 0.0;
+}
+
+// exp(-x) of the Eq. 7 propagator, x = V dt/2.  Ground-state runs have x of a few 1e-2 at most (cfg 2: V < 60,
+// dt/2 = 2.5e-4), where the degree-8 Taylor polynomial is exact to the last bit or two (x^9/9! < 4e-17 for
+// |x| < 1/16) at 8 FMAs; anything larger takes the library routine (a branch, uniform in practice).
+__device__ __forceinline__ double exp_neg(double x) {
+    if (fabs(x) < 0.0625) {
+        const double r = -x;
+        double q = 1.0 / 40320.0;
+        q = fma(q, r, 1.0 / 5040.0);
+        q = fma(q, r, 1.0 / 720.0);
+        q = fma(q, r, 1.0 / 120.0);
+        q = fma(q, r, 1.0 / 24.0);
+        q = fma(q, r, 1.0 / 6.0);
+        q = fma(q, r, 0.5);
+        q = fma(q, r, 1.0);
+        return fma(q, r, 1.0);
+    }
+    return exp(-x);
 }
 
 constexpr int KZMAX = 32;                 // planes per stream (host splits work items to at most this)
@@ -264,6 +292,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
     // halo duty: neighbour tile hq (0..3 = -x,+x,-y,+y), values LPH*e + hj of its 8R-value edge
     const int hq = t / LPH, hj = t % LPH;
     unsigned hbm[NHE], hoff[NHE];
+    int hdr[NHE], hdc[NHE];                                // position of halo value e relative to the tile's (0, 0) column
     bool hhi[NHE];                                         // value e lives in the high mask word
 #pragma unroll
     for (int e = 0; e < NHE; ++e) {
@@ -278,6 +307,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
             nlx = rr; nly = hq == 2 ? 8 - R + cc : cc;
             drow = rr; dcol = hq == 2 ? cc - R : 8 + cc;
         }
+        hdr[e] = drow; hdc[e] = dcol;
         hbm[e] = (1u << ((nlx * 8 + nly) & 31)) - 1u;
         hhi[e] = nlx >= 4;
         hoff[e] = (unsigned)((drow + R) * G::PY + (dcol + R)) * ES;
@@ -301,11 +331,26 @@ stage_kernel(const __grid_constant__ StageParams p) {
             qxy[e] = fma(p.hax, x * x, qy);
         }
     }
+    // K1: the same for the halo values (and the 19-point corner) this lane copies: it applies the Eq. 7 half step to them
+    double qxh[NHE], qxc = 0.0;
+    if (MODE == MODE_KINP) {
+#pragma unroll
+        for (int e = 0; e < NHE; ++e) {
+            const double x = ((double)(w->ix0 + hdr[e]) - p.xc) * p.pot.h + p.pot.cx;
+            const double y = ((double)(w->iy0 + hdc[e]) - p.yc) * p.pot.hy + p.pot.cy;
+            qxh[e] = fma(p.hax, x * x, p.hay * (y * y));
+        }
+        if (HOC) {
+            const double x = ((double)(w->ix0 + ((t & 2) ? 8 : -1)) - p.xc) * p.pot.h + p.pot.cx;
+            const double y = ((double)(w->iy0 + ((t & 1) ? 8 : -1)) - p.yc) * p.pot.hy + p.pot.cy;
+            qxc = fma(p.hax, x * x, p.hay * (y * y));
+        }
+    }
     // everything above read the work record and the slab tables only; psi, the aux operand and the lazy scale are
     // written by the kernels before this one
     asm volatile("griddepcontrol.wait;\n" ::: "memory");
     double sc = 1.0, gsc = p.g;
-    if (MODE == MODE_IMAG || MODE == MODE_PREP) { sc = *p.scale_in; gsc = p.g * (sc * sc); }
+    if (MODE == MODE_IMAG || MODE == MODE_PREP || MODE == MODE_KINP) { sc = *p.scale_in; gsc = p.g * (sc * sc); }
 
     int niter = ne;
     if (SPW == 2) niter = max(niter, __shfl_xor_sync(0xffffffffu, niter, 16));   // both halves run the same loop
@@ -379,10 +424,50 @@ stage_kernel(const __grid_constant__ StageParams p) {
 #pragma unroll
     for (int i = 0; i < PF; ++i) produce(i, (unsigned)i, (unsigned)((i + NAUX - (R % NAUX)) % NAUX));
 
+    // K1: every value this lane copied for plane index j -- its patch, its share of the halo, its
+    // corner -- is replaced in the slot by a = s c exp(-V ca) (1 - g ca |s c|^2) (Eq. 7 with the linearised interaction
+    // factor, the lazy scale s of the previous iteration): the arithmetic of MODE_PREP at the point itself, so the result
+    // does not depend on which tile stages the value; zero-filled points stay zero.  Done one plane step ahead of the
+    // stencil (the copies of plane j have landed for THIS lane after its wait_group; the other lanes see the result
+    // after the next __syncwarp), so that the dependent chain load -> V -> exp -> store overlaps the previous plane's work.
+    auto half_step_plane = [&](const int j, const unsigned sj) {
+        if (j >= ne) return;
+        const double zk = ((double)(kstart + j) - p.zc) * p.pot.hz + p.pot.cz;
+        const double qzk = p.haz * (zk * zk) - p.delta_eff;
+        auto half_step = [&](const C c, const double q) -> C {
+            double vp = q + qzk;
+            if (p.pot.kind == GPE_POT_DRESSED) vp = fast_sqrt(fma(vp, vp, p.om2)) - p.pot.omega;
+            const double c2 = (double)c.x * (double)c.x + (double)c.y * (double)c.y;
+            const T f = (T)(sc * exp_neg(vp * p.ca) * fma(-gsc * p.ca, c2, 1.0));
+            return mk<T>(c.x * f, YV(c.y * f));
+        };
+        const unsigned sa = ring + sj * SLOT_BYTES;
+#pragma unroll
+        for (int e = 0; e < PR; ++e) {
+            const C c = lds_c(sa + own_off + (unsigned)e * ROW_BYTES, (EL*)nullptr);
+            sts_c(sa + own_off + (unsigned)e * ROW_BYTES, half_step(c, qxy[e]), (EL*)nullptr);
+        }
+        if (HOC || (j >= lead && j < ne - R)) {
+#pragma unroll
+            for (int e = 0; e < NHE; ++e) {
+                const C c = lds_c(sa + hoff[e], (EL*)nullptr);
+                sts_c(sa + hoff[e], half_step(c, qxh[e]), (EL*)nullptr);
+            }
+            if (HOC && t < 4) {
+                const C c = lds_c(sa + coff, (EL*)nullptr);
+                sts_c(sa + coff, half_step(c, qxc), (EL*)nullptr);
+            }
+        }
+    };
+    if (MODE == MODE_KINP) {
+        cp_async_wait<PF - 1>();
+        half_step_plane(0, 0u);
+    }
+
     // one plane step at plane index i (plane k = kstart + i).  (PN, AN) = set of plane k-1, (PO, AO) = set of
     // plane k-R (the same set for R = 1).  sl = ring slot of plane i; al = aux slot of plane i - R.
     auto step = [&](C (&PN)[PR], C (&AN)[PR], C (&PO)[PR], C (&AO)[PR], const int i, const unsigned sl, const unsigned al) {
-        cp_async_wait<PF - 1>();
+        if (MODE == MODE_KINP) cp_async_wait<PF - 2>(); else cp_async_wait<PF - 1>();
         __syncwarp();
         {
             unsigned sp = sl + PF, ap = al + PF;
@@ -391,6 +476,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
             produce(i + PF, sp, ap);
         }
         if (i >= ne) return;
+        if (MODE == MODE_KINP) half_step_plane(i + 1, sl + 1 == NSLOT ? 0u : sl + 1);
         const unsigned so = ring + sl * SLOT_BYTES + own_off;   // own patch in the slot of plane k
         const int ic = i - R;                                   // plane finished in this step
         // ---- output plane: activity bits and storage positions --------------------------------------------
@@ -453,7 +539,7 @@ stage_kernel(const __grid_constant__ StageParams p) {
         // ---- V(r,t) of plane c: depends on coordinates only, so its dependency chains (one per patch point,
         //      interleaved) are issued here and overlap the shared-memory latency of psi(k) --------------------
         double vpot[PR];
-        if (cany && MODE != MODE_KIN) {
+        if (cany && MODE != MODE_KIN && MODE != MODE_KINP) {
             const double zc = ((double)(kstart + ic) - p.zc) * p.pot.hz + p.pot.cz;
             const double qz = p.haz * (zc * zc) - p.delta_eff;
 #pragma unroll
@@ -519,16 +605,16 @@ stage_kernel(const __grid_constant__ StageParams p) {
                     acc[3] += (double)a2;
                     continue;
                 }
-                if (MODE == MODE_PREP || MODE == MODE_KIN || MODE == MODE_SPLITB) {
+                if (MODE == MODE_PREP || MODE == MODE_KIN || MODE == MODE_KINP || MODE == MODE_SPLITB) {
                     // the paper's split iteration: Euler half step of the kinetic part and / or the diagonal
                     // propagator exp(-V ca) (1 - g ca |u|^2) of Eq. 7 with the linearised interaction factor
                     const T ca = (T)p.ca;
                     C u = cv;
                     if (MODE != MODE_PREP) u = mk<T>(fma(-ca, tc.x, cv.x), YV(fma(-ca, tc.y, cv.y)));
                     C o = u;
-                    if (MODE != MODE_KIN) {
+                    if (MODE != MODE_KIN && MODE != MODE_KINP) {
                         const double u2 = (double)u.x * (double)u.x + (double)u.y * (double)u.y;
-                        const T f = (T)(sc * exp(-vpot[e] * p.ca) * fma(-gsc * p.ca, u2, 1.0));
+                        const T f = (T)(sc * exp_neg(vpot[e] * p.ca) * fma(-gsc * p.ca, u2, 1.0));
                         o = mk<T>(u.x * f, YV(u.y * f));
                     }
                     if (MODE == MODE_SPLITB) {
@@ -693,6 +779,7 @@ cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
         case MODE_KIN: return launch_one<T, R, MODE_KIN, HOC, false>(p, st);
         case MODE_SPLITB: return launch_one<T, R, MODE_SPLITB, HOC, false>(p, st);
         case MODE_LC: return launch_one<T, R, MODE_LC, HOC, false>(p, st);
+        case MODE_KINP: return launch_one<T, R, MODE_KINP, HOC, false>(p, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -707,6 +794,7 @@ cudaError_t launch_mode_real(int mode, const StageParams& p, cudaStream_t st) {
         case MODE_PREP: return launch_one<double, R, MODE_PREP, HOC, true>(p, st);
         case MODE_KIN: return launch_one<double, R, MODE_KIN, HOC, true>(p, st);
         case MODE_SPLITB: return launch_one<double, R, MODE_SPLITB, HOC, true>(p, st);
+        case MODE_KINP: return launch_one<double, R, MODE_KINP, HOC, true>(p, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -730,6 +818,7 @@ cudaError_t set_attr_modes() {
     if ((e = set_attr<T, R, MODE_KIN, HOC, false>())) return e;
     if ((e = set_attr<T, R, MODE_SPLITB, HOC, false>())) return e;
     if ((e = set_attr<T, R, MODE_LC, HOC, false>())) return e;
+    if ((e = set_attr<T, R, MODE_KINP, HOC, false>())) return e;
     return cudaSuccess;
 }
 template <int R, bool HOC>
@@ -741,6 +830,7 @@ cudaError_t set_attr_modes_real() {
     if ((e = set_attr<double, R, MODE_PREP, HOC, true>())) return e;
     if ((e = set_attr<double, R, MODE_KIN, HOC, true>())) return e;
     if ((e = set_attr<double, R, MODE_SPLITB, HOC, true>())) return e;
+    if ((e = set_attr<double, R, MODE_KINP, HOC, true>())) return e;
     return cudaSuccess;
 }
 

@@ -190,6 +190,31 @@ def test_imag_split_small_shell(P, stencil, dtype):
         assert sim.energy()["total"] < e0
 
 
+@pytest.mark.parametrize("dtype", ["complex128", "complex64", "float64"])
+@pytest.mark.parametrize("stencil", [7, 13, 19])
+def test_imag_split_k1_equals_three_launches(P, stencil, dtype, monkeypatch):
+    """The paper's K1 (Eq. 7 half step and lazy scale applied to every value while it is staged, own
+    and halo, then the first Euler half step) gives bit for bit what the separate pointwise launch followed by the
+    kinetic launch gives (GPE_K1=0): the same arithmetic at the same point, whichever tile stages the value."""
+    w = I.small_shell(40, stencil, "complex128" if dtype == "float64" else dtype).with_(g=400.0)
+    box, pot, act = oracle_objs(w)
+    grid = P.Grid.from_workload(w)
+    psi = I.make_psi0(w, act)
+    psi = np.abs(psi).astype(np.float64) if dtype == "float64" else psi.astype(np.complex64 if dtype == "complex64" else np.complex128)
+    out = []
+    for k1 in ("1", "0"):
+        monkeypatch.setenv("GPE_K1", k1)
+        sim = P.Sim(grid, dtype, stencil, w.g)
+        sim.set_psi_host(psi)
+        n0 = sim.kernel_launches
+        sim.run_imag_split(2e-3, 6)
+        out.append((sim.get_psi_host().copy(), sim.kernel_launches - n0))
+        sim.close()
+    assert np.array_equal(out[0][0], out[1][0])
+    assert np.all(np.isfinite(out[0][0].view(np.float64 if dtype != "complex64" else np.float32)))
+    assert out[1][1] - out[0][1] == 6          # one stencil launch less per iteration
+
+
 @pytest.mark.parametrize("dtype", ["complex128", "complex64"])
 def test_regrid_remap(P, dtype):
     """Re-gridding between ramp stages: the state is carried from the shell at Delta = 14 to the

@@ -215,6 +215,34 @@ def test_imag_split_k1_equals_three_launches(P, stencil, dtype, monkeypatch):
     assert out[1][1] - out[0][1] == 6          # one stencil launch less per iteration
 
 
+@pytest.mark.parametrize("dims,p,seed", [((9, 7, 11), 0.4, 3), ((17, 16, 40), 0.15, 4), ((8, 8, 70), 0.9, 5),
+                                         ((6, 6, 6), 1.1, 6), ((19, 21, 37), 0.6, 8), ((1, 20, 33), 0.8, 9), ((24, 1, 1), 0.7, 10)])
+@pytest.mark.parametrize("stencil", [7, 13, 19])
+@pytest.mark.parametrize("kz", [32, 3, 1])
+def test_imag_split_k1_random_masks(P, dims, p, seed, stencil, kz, monkeypatch):
+    """K1 on random masks (holes everywhere, box faces touched, streams of 1-3 planes, boxes one point thick): the
+    iteration against the oracle, and bit for bit against the three-launch form."""
+    nx, ny, nz = dims
+    w = I.Workload(name="rnd", nx=nx, ny=ny, nz=nz, h=0.3, kind=I.DRESSED, ax=1.0, ay=0.7, az=1.2, delta0=2.0,
+                   delta1=2.0, omega=1.5, stencil=stencil, g=3.0)
+    act = I.random_mask_lin(seed, nx, ny, nz, p)
+    box, pot, act = oracle_objs(w, act)
+    grid = P.Grid.from_workload(w, active=act)
+    og = O.SparseGrid(box, act, RADIUS[stencil])
+    psi = I.random_psi(seed + 100, act.size)
+    out = []
+    for k1 in ("1", "0"):
+        monkeypatch.setenv("GPE_K1", k1)
+        sim = P.Sim(grid, "complex128", stencil, w.g)
+        sim.set_planes_per_block(kz)
+        sim.set_psi_host(psi)
+        sim.run_imag_split(5e-3, 4)
+        out.append(sim.get_psi_host().copy())
+        sim.close()
+    assert np.array_equal(out[0], out[1])
+    assert rel_max(out[0], O.run_imag_split(og, pot, w.g, 0.0, 5e-3, 4, psi, stencil)) < 1e-12
+
+
 @pytest.mark.parametrize("dtype", ["complex128", "complex64"])
 def test_regrid_remap(P, dtype):
     """Re-gridding between ramp stages: the state is carried from the shell at Delta = 14 to the

@@ -590,8 +590,11 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     s->csize = dtype == GPE_C128 ? 16 : 8;
     s->n = g->h.n_active;
     // planes per stream: small grids are cut into shorter streams so that every SM holds several
-    // (measured on B200: 67 k points best at 4, 1.2 M at 8, 1e7 at 16 or more)
+    // (measured on B200: 67 k points best at 4, 1.2 M at 8, 1e7 at 16; from 2e7 points on the 13- / 19-point kernels
+    // are best at 32, the 7-point kernels, whose streams are long runs of cheap planes, at 24: cfg 3a 0.82 of the copy
+    // rate against 0.78 at 32; profiles/r2_experiments.md 6.9)
     s->kz = s->n < 300000 ? 4 : s->n < 3000000 ? 8 : s->n < 20000000 ? 16 : 32;
+    if (s->kz == 32 && !s->hoc && s->radius == 1) s->kz = 24;
     for (int k = 0; k < 4; ++k) s->buf[k] = (char*)dev_state + k * bb;
     s->staging = (char*)dev_state + 4 * bb;
     cudaError_t e = cudaMalloc(&s->d_sums, (NACC + 2) * sizeof(double));

@@ -29,7 +29,8 @@
 // stencil, PAPER.md:341-343 Eq. B2: diagonal-tile tables, corner halo, in-plane face / diagonal sums carried
 // along z), per-axis weights for anisotropic grids (Eq. B1), T = float / double, REAL (8-byte real-valued
 // state for ground states), and the MODEs of gpe_internal.h: operator, RK stages S1-S4 and the
-// general stage LC of Eq. A6-A7 (RKHE3, RKCK), Euler imaginary time, the paper's split iteration, energy sums.
+// general stage LC of Eq. A6-A7 (RKHE3, RKCK), Euler imaginary time, the paper's split iteration (K1 = KINP: the
+// Eq. 7 half step applied to every staged value inside the kinetic kernel; K2 = SPLITB), energy sums.
 #include <cuda_runtime.h>
 
 #include <cstdint>

@@ -218,6 +218,7 @@ __global__ void __launch_bounds__(STAGE_THREADS, 16)
 stage_kernel(const __grid_constant__ StageParams p) {
     static_assert(!HOC || (R == 1 && PR == 2), "the 19-point stencil has radius 1 and runs with a warp per stream");
     static_assert(!REAL || sizeof(T) == 8, "the real-valued state is fp64");
+    static_assert(MODE != MODE_KINP || pf_of(R) >= 2, "K1 works on the plane after the current one: two planes must have landed");
     using C = typename CxOf<T>::type;                      // value in registers
     using EL = typename ElemOf<T, REAL>::type;             // value in memory
     constexpr bool HAS_AUX = mode_has_aux(MODE);

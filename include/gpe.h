@@ -246,6 +246,44 @@ int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 int gpe_norm(gpe_sim* s, double* out_host, void* stream);
 int gpe_energy(gpe_sim* s, gpe_energy_out* out_host, void* stream);
 
+/* a6 without any allocation: *dev_out = cell_volume * sum_{k<n} |dev_psi[k]|^2  (Eq. 3; the sum of the
+ * paper's kernel K3), fp64 accumulation in a fixed order (the same array gives the same bits every time),
+ * asynchronous on `stream`.  The order of the values does not matter to the sum, so canonical order, a sim's storage
+ * order or any other arrangement of the wavefunction will do.
+ *
+ * Why it exists.  gpe_norm needs a gpe_sim, and a sim costs four cudaMalloc calls and one cudaMallocHost.  Some
+ * callers cannot have that happen: a process whose framework allocator (torch's caching allocator, typically) already
+ * holds almost all device memory for 1e8-point state blocks, where a raw cudaMalloc made by a library fails although
+ * the framework still has room; a norm check placed between time steps while other streams are busy, where cudaMalloc /
+ * cudaFree would wait for the whole device on every call; code that has only an array of values (a checkpoint reader,
+ * a diagnostic thread) and no grid or sim.  This call makes no cudaMalloc, cudaFree, cudaMallocHost or other allocating
+ * call, now or later, and creates no stream or event.  The block partial sums go to a fixed array compiled into the
+ * library: every GPU that loads the library's kernels holds GPE_NORM_NOALLOC_SCRATCH_BYTES for it until the process
+ * exits, whether this function is called or not.
+ *
+ * Arguments.  dev_psi: n values on the current CUDA device (device or managed memory; may be NULL when n = 0), aligned
+ * to their size: interleaved complex128 (GPE_C128), interleaved complex64 (GPE_C64) or real doubles (GPE_R64).
+ * cell_volume: h hy hz of the grid (finite, > 0).  dev_out: one double on the same device, caller-owned, written by the
+ * last kernel; read it after synchronising `stream` (or from later work on `stream`).  n = 0 writes 0.
+ *
+ * Limits and rules.
+ *   - n <= GPE_NORM_NOALLOC_MAX_VALUES (2^29 = 536 870 912: one scratch slot per 8192 values); a larger n returns
+ *     GPE_ERR_UNSUPPORTED and launches nothing.  For complex states of up to 19 398 656 values the summation order is
+ *     the one gpe_norm uses on the same array; above that gpe_norm caps its block count, and for GPE_R64 it sums pairs,
+ *     so there the two agree to rounding only.
+ *   - The first call on each device looks up the scratch array's address on that device (which can also be the moment
+ *     the CUDA runtime loads the library's kernels there).  Make that first call during start-up, with the device
+ *     current, before any stream capture begins; later calls on that device only launch two kernels.
+ *   - All calls on one device share the scratch.  It needs no clearing (a call overwrites every slot it later reads),
+ *     but two calls whose kernels can overlap on the GPU -- different streams without an ordering between them, or
+ *     different host threads -- corrupt each other's sums.  Calls queued on one stream are safe.
+ *   - The device that owns dev_psi and dev_out must be current; otherwise INVALID_ARG.
+ * Errors: INVALID_ARG (null or misaligned pointer, pointer not on the current device, n < 0, unknown dtype, bad
+ * cell_volume), UNSUPPORTED (n over the limit, device ordinal above 63), CUDA. */
+#define GPE_NORM_NOALLOC_SCRATCH_BYTES 524288
+#define GPE_NORM_NOALLOC_MAX_VALUES 536870912LL
+int gpe_norm_noalloc(const void* dev_psi, int64_t n, int dtype, double cell_volume, double* dev_out, void* stream);
+
 /* Number of kernels this sim has launched so far (bench.py's gpu_launches). */
 int gpe_sim_kernel_launches(const gpe_sim* s, int64_t* out);
 /* Name/duration of the stage kernels: enables CUDA-event timing of every RK4 stage launch inside

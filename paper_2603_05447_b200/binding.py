@@ -64,7 +64,10 @@ SYMBOLS = (
     "gpe_run_imag", "gpe_norm", "gpe_energy", "gpe_sim_kernel_launches", "gpe_sim_time_stages",
     "gpe_sim_stage_time_ms", "gpe_sim_set_planes_per_block", "gpe_imag_split_step", "gpe_run_imag_split",
     "gpe_remap_psi", "gpe_step_rkhe3", "gpe_run_rkhe3", "gpe_step_rkck", "gpe_run_rkck", "gpe_sim_set_compact_weights",
+    "gpe_norm_noalloc",
 )
+
+NORM_NOALLOC_MAX_VALUES = 1 << 29       # GPE_NORM_NOALLOC_MAX_VALUES
 
 _lib = None
 
@@ -173,6 +176,29 @@ def _stream_ptr(stream=None):
     import torch
     st = stream if stream is not None else torch.cuda.current_stream()
     return C.c_void_p(st.cuda_stream)
+
+
+def norm_noalloc(psi_dev, cell_volume: float, out_dev, stream=None, n=None):
+    """gpe_norm_noalloc: out_dev[0] = cell_volume * sum |psi_dev[k]|^2 without a Sim and without any allocation.
+
+    For programs that cannot let the library call cudaMalloc: all device memory already belongs to torch's caching
+    allocator, or the check runs between time steps while other streams must not be stalled, or there is only an array
+    and no Sim.  The caller supplies both tensors (this wrapper creates none): psi_dev a contiguous CUDA tensor of
+    complex128, complex64 or float64 values in any order, out_dev a one-element float64 CUDA tensor on the same device,
+    which must be the current one.  Asynchronous on `stream`: synchronise before reading out_dev.  At most
+    NORM_NOALLOC_MAX_VALUES values (2^29); more raises GpeError(GPE_ERR_UNSUPPORTED).  Calls share one scratch array
+    inside the library, so do not let two of them run concurrently on one GPU; make the first call on a device during
+    start-up (it resolves the scratch address).  `n` (default: psi_dev.numel()) only exists so that the size check can be
+    exercised without allocating 2^29 values."""
+    name = str(psi_dev.dtype).replace("torch.", "")
+    code = {"complex128": C128, "complex64": C64, "float64": R64}.get(name)
+    if code is None:
+        raise ValueError(f"psi_dev must be complex128, complex64 or float64, not {psi_dev.dtype}")
+    assert psi_dev.is_cuda and psi_dev.is_contiguous()
+    assert out_dev.is_cuda and out_dev.numel() == 1 and str(out_dev.dtype) == "torch.float64"
+    _check(lib().gpe_norm_noalloc(C.c_void_p(psi_dev.data_ptr()), C.c_int64(psi_dev.numel() if n is None else n),
+                                  C.c_int(code), C.c_double(cell_volume), C.c_void_p(out_dev.data_ptr()),
+                                  _stream_ptr(stream)))
 
 
 class Sim:

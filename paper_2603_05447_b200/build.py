@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libgpe_b200.so")
-SOURCES = ["gpe_layout.cpp", "gpe_kernels.cu", "gpe_stage.cu", "gpe_api.cu"]
+SOURCES = ["gpe_layout.cpp", "gpe_kernels.cu", "gpe_stage.cu", "gpe_api.cu", "gpe_noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "gpe_internal.h"), os.path.join(INCLUDE, "gpe.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 

@@ -446,6 +446,11 @@ int sums_to_host(gpe_sim* s, double out[NACC], void* stream) {
 
 }  // namespace
 
+namespace gpe {
+int api_fail(int code, const char* msg) { return fail(code, msg); }
+int api_cuda_fail(int cuda_error, const char* what) { return cuda_fail((cudaError_t)cuda_error, what); }
+}  // namespace gpe
+
 extern "C" {
 
 const char* gpe_last_error(void) { return g_err.c_str(); }

@@ -166,4 +166,9 @@ int launch_scale(int dtype, void* storage, int64_t n, const double* scale, void*
 int launch_set_scalar(double* dst, double v, void* stream);
 int kernels_configure();  // sets max dynamic shared memory attributes once; returns cudaError_t
 
+// Error text for entry points that live outside gpe_api.cu (gpe_noalloc.cu): store the calling thread's
+// gpe_last_error() text and return `code` (api_fail) or GPE_ERR_CUDA (api_cuda_fail, text = what + the CUDA error string).
+int api_fail(int code, const char* msg);
+int api_cuda_fail(int cuda_error, const char* what);
+
 }  // namespace gpe

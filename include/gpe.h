@@ -158,7 +158,9 @@ int gpe_sim_state_bytes(const gpe_grid* g, int dtype, size_t* out);
  * edges 1/6h^2; radius 1 plus the twelve edge neighbours, zero outside M like every other read), or 27 (3x3x3
  * compact stencil with caller-supplied weights, gpe_sim_set_compact_weights).
  * g: interaction strength multiplying |psi|^2; n_target: value of h^3 sum|psi|^2 that imaginary-time
- * steps renormalise to (Eq. 3).  dev_state: device memory, 256-byte aligned, >= state_bytes,
+ * steps renormalise to (Eq. 3).  dev_state: memory of the current device (cudaMalloc / a framework
+ * allocator) or managed memory (cudaMallocManaged), 256-byte aligned, >= state_bytes, checked before anything is
+ * allocated (INVALID_ARG);
  * must stay valid until gpe_sim_destroy; it is zero-initialised here (psi = 0, t = 0).  Uploads the
  * grid's tables to the current CUDA device on first use.  Errors: INVALID_ARG, UNSUPPORTED (tile shape
  * other than 8x8, halo_width < radius), CUDA (no device, not sm_100), OUT_OF_MEMORY. */
@@ -185,8 +187,10 @@ int gpe_apply_H(gpe_sim* s, double t, const void* dev_in_canonical, void* dev_ou
  * t, t+dt/2, t+dt/2, t+dt.  Step n of a run starts at t_start + n*dt (a product, not a running sum); the
  * sim clock ends at t_start + nsteps*dt.  Asynchronous on `stream`.  Runs of 16 or more steps on grids below 4e6
  * points whose potential does not change during the run are replayed from a CUDA graph of 8 steps that the library
- * captures on a stream of its own (same kernels, parameters and order: bit-identical results; the environment
- * variable GPE_GRAPH=0 turns it off, GPE_PDL=0 turns off programmatic dependent launch of the stage kernels). */
+ * captures on a stream of its own (same kernels, parameters and order: bit-identical results;
+ * gpe_sim_set_option(GPE_OPT_RK4_GRAPH, 0) turns it off, GPE_OPT_PDL = 0 turns off programmatic dependent launch of
+ * the stage kernels).  If `stream` is itself being captured the library opens no capture of its own and the steps are
+ * enqueued one by one. */
 int gpe_step_rk4(gpe_sim* s, double dt, void* stream);
 int gpe_run_rk4(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 
@@ -211,7 +215,16 @@ int gpe_run_rkck(gpe_sim* s, double dt, int64_t nsteps, void* stream);
  * clock (PAPER.md:35, :60 Eq. 6, :87; forward-Euler reading DESIGN.md R7).  One fused kernel per step
  * (update + block partial sums) + a one-block finalise; the scale is applied lazily at the next load as
  * in the paper's kernel K1 and flushed at the end of the call, so the state seen by every
- * other call is normalised.  A state with zero norm yields GPE_ERR_STATE at the next host-scalar call. */
+ * other call is normalised.
+ * Degenerate states.  If the particle number becomes zero or non-finite during a run, no renormalisation is applied
+ * (the values stay as they are, no NaN is manufactured) and a flag is raised on the device.  The runs are asynchronous,
+ * so the flag is reported later, once, as GPE_ERR_STATE, by the first of these calls that follows the run: gpe_norm,
+ * gpe_energy, gpe_get_psi_host (after their synchronisation; the out-parameters of gpe_norm / gpe_energy are not
+ * written, the host array of gpe_get_psi_host is), or gpe_run_imag / gpe_run_imag_split / their single-step forms
+ * (checked on entry without waiting: if the earlier run has finished and raised the flag, the new run is not enqueued).
+ * The Runge-Kutta calls, gpe_apply_H and the device-side gpe_get_psi never report it.  Replacing the state -- gpe_set_psi,
+ * gpe_set_psi_host, gpe_remap_psi into the sim -- discards a flag that has not been reported yet: it belonged to the
+ * state that is gone (enqueue the replacement on the stream of the run, or ordered after it). */
 int gpe_imag_step(gpe_sim* s, double dt, void* stream);
 int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream);
 
@@ -221,7 +234,12 @@ int gpe_run_imag(gpe_sim* s, double dt, int64_t nsteps, void* stream);
  * dropped are lost (the caller checks gpe_norm(dst) and picks the cutoff, e.g. the paper's 5 max(mu_i, mu_i+1)).
  * Both sims must have the same precision and grids post-selected from the same bounding box (nx, ny, nz, h,
  * center), else INVALID_ARG.  dst's clock is set to src's.  The index match is one merge pass on the host over
- * the two ascending index lists; the values move on the device (unpack, gather, pack).  Synchronises `stream`. */
+ * the two ascending index lists; the table is copied to the device and the values move there (unpack, gather, pack),
+ * all enqueued on `stream`: the call does not wait for them.  Each destination sim keeps ONE device table and one
+ * staging area for remaps into it, so remaps into the same dst (and other calls that use dst's staging: the *_host
+ * copies, gpe_apply_H) must be issued on one stream or otherwise ordered; src's staging area is used too.  `stream`
+ * must not be in capture (UNSUPPORTED: the table comes from pageable host memory).  The first remap into a sim
+ * allocates the table (OUT_OF_MEMORY if that fails). */
 int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream);
 
 /* a5 (second mode): the paper's own ground-state iteration, in its order (PAPER.md:60-67,
@@ -234,8 +252,8 @@ int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream);
  * Two stencil launches per iteration, as the paper's K1 / K2 (:87): K1 applies Eq. 7 and the lazily applied scale of
  * the previous iteration to every value while it is staged for the stencil (own and halo) and takes the first Euler
  * half step; K2 takes the second Euler half step, applies Eq. 7 and writes block partial sums; then a one-block
- * finalise.  exp(-V dt/2) is evaluated analytically per value (no propagator array is read).  GPE_K1=0 in the
- * environment (read per call) runs the bit-identical three-launch form (pointwise Eq. 7, Euler half step, Euler half
+ * finalise.  exp(-V dt/2) is evaluated analytically per value (no propagator array is read).  gpe_sim_set_option(GPE_OPT_FUSED_K1,
+ * 0) runs the bit-identical three-launch form (pointwise Eq. 7, Euler half step, Euler half
  * step + Eq. 7).  The scale is flushed at the end of the call.
  * With a GPE_R64 sim the state is real (:67).  Same arguments and errors as gpe_run_imag. */
 int gpe_imag_split_step(gpe_sim* s, double dt, void* stream);
@@ -299,6 +317,21 @@ int gpe_sim_stage_time_ms(gpe_sim* s, double ms_out[4], int64_t count_out[4]);
  * Eq. B2 (corner 0), i.e. it equals stencil 19.  Also valid on a stencil-19 sim.  STATE for the star stencils. */
 int gpe_sim_set_compact_weights(gpe_sim* s, double centre, const double* face_xyz, const double* edge_xy_xz_yz,
                                 double corner);
+
+/* Switches between forms of the same computation that give bit-identical results (tested); value 0 or 1, all default
+ * to 1; a sim-level setting, read by every later call on the sim.  The library reads no environment variable.
+ *   GPE_OPT_FUSED_K1   gpe_run_imag_split: 1 = the paper's K1 / K2 pair (two stencil launches per iteration),
+ *                      0 = three launches (pointwise Eq. 7, Euler half step, Euler half step + Eq. 7).
+ *   GPE_OPT_RK4_GRAPH  gpe_run_rk4: 1 = long runs on small grids in a static potential replay a captured CUDA graph,
+ *                      0 = every step is enqueued launch by launch.
+ *   GPE_OPT_PDL        1 = the stage kernels are launched with programmatic dependent launch (the next launch's
+ *                      prologue overlaps the tail of the previous one), 0 = plain stream-ordered launches.  Changing it
+ *                      drops the captured RK4 graph (waits for the device first).
+ * Errors: INVALID_ARG (null sim, unknown option, value other than 0 / 1). */
+#define GPE_OPT_FUSED_K1 0
+#define GPE_OPT_RK4_GRAPH 1
+#define GPE_OPT_PDL 2
+int gpe_sim_set_option(gpe_sim* s, int option, int value);
 
 /* Tuning knob: planes per thread block (1..32, default chosen per dtype/stencil).  INVALID_ARG otherwise. */
 int gpe_sim_set_planes_per_block(gpe_sim* s, int kz);

@@ -17,6 +17,7 @@ from . import build as _build
 HARMONIC, DRESSED = 0, 1
 MASK_AT_DELTA0, MASK_AT_DELTA1, MASK_UNION = 0, 1, 2
 C64, C128, R64 = 0, 1, 2
+OPT_FUSED_K1, OPT_RK4_GRAPH, OPT_PDL = 0, 1, 2
 
 ERR_NAMES = {-1: "GPE_ERR_INVALID_ARG", -2: "GPE_ERR_OUT_OF_MEMORY", -3: "GPE_ERR_CUDA",
              -4: "GPE_ERR_UNSUPPORTED", -5: "GPE_ERR_STATE"}
@@ -64,7 +65,7 @@ SYMBOLS = (
     "gpe_run_imag", "gpe_norm", "gpe_energy", "gpe_sim_kernel_launches", "gpe_sim_time_stages",
     "gpe_sim_stage_time_ms", "gpe_sim_set_planes_per_block", "gpe_imag_split_step", "gpe_run_imag_split",
     "gpe_remap_psi", "gpe_step_rkhe3", "gpe_run_rkhe3", "gpe_step_rkck", "gpe_run_rkck", "gpe_sim_set_compact_weights",
-    "gpe_norm_noalloc",
+    "gpe_norm_noalloc", "gpe_sim_set_option",
 )
 
 NORM_NOALLOC_MAX_VALUES = 1 << 29       # GPE_NORM_NOALLOC_MAX_VALUES
@@ -355,6 +356,10 @@ class Sim:
         f = (C.c_double * 3)(*face)
         e = (C.c_double * 3)(*edge)
         _check(lib().gpe_sim_set_compact_weights(self._h, C.c_double(centre), f, e, C.c_double(corner)))
+
+    def set_option(self, option: int, value: int):
+        """gpe_sim_set_option: OPT_FUSED_K1 / OPT_RK4_GRAPH / OPT_PDL, value 0 or 1 (bit-identical forms of the same path)."""
+        _check(lib().gpe_sim_set_option(self._h, C.c_int(option), C.c_int(value)))
 
     def set_planes_per_block(self, kz: int):
         _check(lib().gpe_sim_set_planes_per_block(self._h, C.c_int(kz)))

@@ -47,10 +47,15 @@ struct gpe_sim {
     double* h_flag = nullptr;   // pinned copy of the degenerate-norm flag, filled asynchronously at the end of a run
     cudaEvent_t ev_flag = nullptr;
     bool flag_pending = false;
+    void* flag_stream = nullptr;   // stream of the run whose flush recorded ev_flag (the device-side reset goes there)
     // CUDA graph of RK4_GRAPH_STEPS steps for runs on small grids in a potential that does not change during the run
     cudaStream_t cap_stream = nullptr;
     cudaGraphExec_t rk4_exec = nullptr;
-    bool graph_off = false;     // capture failed once, or GPE_GRAPH=0
+    bool graph_off = false;     // capture failed once
+    // gpe_sim_set_option
+    int opt_k1 = 1;             // GPE_OPT_FUSED_K1
+    int opt_graph = 1;          // GPE_OPT_RK4_GRAPH
+    int opt_pdl = 1;            // GPE_OPT_PDL
     struct GraphKey {
         double dt = 0.0, delta = 0.0, g = 0.0, w27[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         void* buf[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -289,11 +294,11 @@ int stage(gpe_sim* s, int mode, double t, double ca, const void* in, const void*
             v.push_back(e);
         }
         CU(cudaEventRecord(v[u], st));
-        KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, mode, p, stream));
+        KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, mode, p, stream, s->opt_pdl));
         CU(cudaEventRecord(v[u + 1], st));
         u += 2;
     } else {
-        KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, mode, p, stream));
+        KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, mode, p, stream, s->opt_pdl));
     }
     if (s->n_blocks > 0) s->launches += 1;
     return GPE_OK;
@@ -330,7 +335,7 @@ int stage_lc(gpe_sim* s, double t, double ca, const void* in, int n_aux, const v
     p.n_aux = n_aux;
     p.coefc = coefc;
     for (int j = 0; j < n_aux; ++j) { p.auxn[j] = aux[j]; p.coef[j] = coef[j]; }
-    KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, MODE_LC, p, stream));
+    KL(launch_stage(s->dtype, s->hoc ? 3 : s->radius, MODE_LC, p, stream, s->opt_pdl));
     if (s->n_blocks > 0) s->launches += 1;
     return GPE_OK;
 }
@@ -366,11 +371,22 @@ int flush_scale(gpe_sim* s, void* stream) {
     CU(cudaMemcpyAsync(s->h_flag, s->d_sums + NACC + 1, sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
     CU(cudaEventRecord(s->ev_flag, (cudaStream_t)stream));
     s->flag_pending = true;
+    s->flag_stream = stream;
+    return GPE_OK;
+}
+
+// The state the deferred degenerate-norm flag referred to has just been replaced (gpe_set_psi, gpe_set_psi_host,
+// gpe_remap_psi into this sim) by work enqueued on `stream`: forget the flag, on the host and -- ordered after the
+// run on the caller's stream, like the new state itself -- on the device.
+int drop_flag(gpe_sim* s, void* stream) {
+    if (!s->flag_pending) return GPE_OK;
+    s->flag_pending = false;
+    CU(cudaMemsetAsync(s->d_sums + NACC + 1, 0, sizeof(double), (cudaStream_t)stream));
     return GPE_OK;
 }
 
 // synced = the caller has just synchronised the stream the run was enqueued on
-int check_flag(gpe_sim* s, bool synced, void* stream) {
+int check_flag(gpe_sim* s, bool synced, void* /*stream of the reporting call*/) {
     if (!s->flag_pending) return GPE_OK;
     if (!synced) {
         cudaError_t q = cudaEventQuery(s->ev_flag);
@@ -382,7 +398,7 @@ int check_flag(gpe_sim* s, bool synced, void* stream) {
     s->flag_pending = false;
     if (*s->h_flag != 0.0) {
         *s->h_flag = 0.0;
-        CU(cudaMemsetAsync(s->d_sums + NACC + 1, 0, sizeof(double), (cudaStream_t)stream));
+        CU(cudaMemsetAsync(s->d_sums + NACC + 1, 0, sizeof(double), (cudaStream_t)s->flag_stream));
         return fail(GPE_ERR_STATE, "the particle number became zero or non-finite during an imaginary-time run (no renormalisation was applied)");
     }
     return GPE_OK;
@@ -398,8 +414,20 @@ constexpr int64_t GRAPH_MAX_POINTS = 4000000;   // above this the stage kernels 
 // caller runs everything step by step); results are bit-identical to the step-by-step path (same kernels, same
 // parameters, same order).
 int64_t rk4_graph_steps(gpe_sim* s, double t0, double dt, int64_t nsteps, void* stream) {
-    static const bool env_off = [] { const char* e = getenv("GPE_GRAPH"); return e && atoi(e) == 0; }();
-    if (env_off || s->graph_off || s->timing || s->n_blocks <= 0 || s->n > GRAPH_MAX_POINTS || nsteps < 2 * RK4_GRAPH_STEPS) return 0;
+    if (!s->opt_graph || s->graph_off || s->timing || s->n_blocks <= 0 || s->n > GRAPH_MAX_POINTS || nsteps < 2 * RK4_GRAPH_STEPS) return 0;
+    {
+        // the caller's stream is itself being captured: this call must not open a capture of its own or instantiate a
+        // graph in the middle of it; the step-by-step launches below go into the caller's capture like any other work
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing((cudaStream_t)stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+            cudaGetLastError();
+            return 0;
+        }
+    }
+    // The replayed launches carry the parameters of the capture, so everything a stage launch depends on must either be
+    // in GraphKey or be constant for the sim's lifetime.  Today the ONLY time dependence of the path is Delta(t) of the
+    // dressed potential (delta_of_t), and Delta(t) is monotone in t, so "equal at both ends of the run" means "constant
+    // over the run".  Any new time-dependent term of V (or a non-monotone ramp) must join GraphKey and this test.
     const gpe_potential& pot = s->grid->h.pot;
     const double d0 = delta_of_t(pot, t0), d1 = delta_of_t(pot, t0 + (double)nsteps * dt);
     if (pot.kind == GPE_POT_DRESSED && d0 != d1) return 0;   // Delta(t) is monotone: equal ends = constant in between
@@ -569,21 +597,23 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     if (((uintptr_t)dev_state & 255) != 0) return fail(GPE_ERR_INVALID_ARG, "dev_state must be 256-byte aligned");
     const size_t bb = buf_bytes(g->h.n_active, dtype);
     if (state_bytes < 5 * bb) return fail(GPE_ERR_INVALID_ARG, "state_bytes too small (see gpe_sim_state_bytes)");
-    int rc = upload_grid(g);
-    if (rc) return rc;
     {
-        // the grid's tables live on the device that was current when its first sim was created: every sim on the
-        // grid, and its state buffer, must be on that device
+        // Checked before anything is allocated.  The grid's tables live on the device that was current when its first
+        // sim was created (upload_grid below, if this is the first): every sim on the grid, and its state buffer, must
+        // be on that device.  The state may be device memory of that device or managed memory.
         int dev = -1;
         CU(cudaGetDevice(&dev));
-        if (dev != g->device) return fail(GPE_ERR_STATE, "the current device is not the one the grid's tables were uploaded to");
+        if (g->on_device && dev != g->device) return fail(GPE_ERR_STATE, "the current device is not the one the grid's tables were uploaded to");
         cudaPointerAttributes attr;
         cudaError_t pe = cudaPointerGetAttributes(&attr, dev_state);
-        if (pe != cudaSuccess || attr.type != cudaMemoryTypeDevice || attr.device != g->device) {
+        const bool ok = pe == cudaSuccess && (attr.type == cudaMemoryTypeManaged || (attr.type == cudaMemoryTypeDevice && attr.device == dev));
+        if (!ok) {
             cudaGetLastError();
-            return fail(GPE_ERR_INVALID_ARG, "dev_state is not device memory of the grid's device");
+            return fail(GPE_ERR_INVALID_ARG, "dev_state is neither device memory of the current (= the grid's) device nor managed memory");
         }
     }
+    int rc = upload_grid(g);
+    if (rc) return rc;
     gpe_sim* s = new (std::nothrow) gpe_sim();
     if (!s) return fail(GPE_ERR_OUT_OF_MEMORY, "host allocation");
     s->grid = g;
@@ -597,7 +627,7 @@ int gpe_sim_create(gpe_grid* g, int dtype, int stencil, double g_int, double n_t
     // planes per stream: small grids are cut into shorter streams so that every SM holds several
     // (measured on B200: 67 k points best at 4, 1.2 M at 8, 1e7 at 16; from 2e7 points on the 13- / 19-point kernels
     // are best at 32, the 7-point kernels, whose streams are long runs of cheap planes, at 24: cfg 3a 0.82 of the copy
-    // rate against 0.78 at 32; profiles/r2_experiments.md 6.9)
+    // rate against 0.78 at 32; round-2 builder's notes, variants not in the tree 6.9)
     s->kz = s->n < 300000 ? 4 : s->n < 3000000 ? 8 : s->n < 20000000 ? 16 : 32;
     if (s->kz == 32 && !s->hoc && s->radius == 1) s->kz = 24;
     for (int k = 0; k < 4; ++k) s->buf[k] = (char*)dev_state + k * bb;
@@ -644,7 +674,7 @@ int gpe_set_psi(gpe_sim* s, const void* dev_psi_canonical, void* stream) {
     if (!s || (!dev_psi_canonical && s->n > 0)) return fail(GPE_ERR_INVALID_ARG, "null argument");
     KL(launch_pack(copy_dtype(s->dtype), dev_psi_canonical, s->buf[0], s->grid->d_perm, s->n, stream));
     if (s->n > 0) s->launches += 1;
-    return GPE_OK;
+    return drop_flag(s, stream);
 }
 
 int gpe_get_psi(gpe_sim* s, void* dev_psi_canonical, void* stream) {
@@ -661,6 +691,13 @@ int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream) {
     if (a.nx != b.nx || a.ny != b.ny || a.nz != b.nz || a.h != b.h || a.hy != b.hy || a.hz != b.hz || a.center[0] != b.center[0] ||
         a.center[1] != b.center[1] || a.center[2] != b.center[2])
         return fail(GPE_ERR_INVALID_ARG, "the two grids must be post-selected from the same bounding box");
+    {
+        // the index table is built on the host and copied from pageable memory: that cannot go into a stream capture
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing((cudaStream_t)stream, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
+        if (cs != cudaStreamCaptureStatusNone)
+            return fail(GPE_ERR_UNSUPPORTED, "gpe_remap_psi cannot be part of a stream capture (it uploads a host-built index table)");
+    }
     dst->t = src->t;
     if (dst->n == 0) return GPE_OK;
     // new canonical rank -> old canonical rank (both index lists ascend: one merge pass), -1 = new point
@@ -684,7 +721,7 @@ int gpe_remap_psi(gpe_sim* src, gpe_sim* dst, void* stream) {
     KL(launch_pack(copy_dtype(dst->dtype), dst->staging, dst->buf[0], dst->grid->d_perm, dst->n, stream));
     src->launches += src->n > 0 ? 1 : 0;
     dst->launches += 2;
-    return GPE_OK;
+    return drop_flag(dst, stream);
 }
 
 int gpe_set_psi_host(gpe_sim* s, const void* host_psi_canonical, void* stream) {
@@ -817,8 +854,7 @@ int gpe_run_imag_split(gpe_sim* s, double dt, int64_t nsteps, void* stream) {
     { int rcf = check_flag(s, false, stream); if (rcf) return rcf; }
     const double h3 = cell_volume(s->grid->h.box);
     const double hdt = 0.5 * dt;
-    const char* k1env = getenv("GPE_K1");                   // GPE_K1=0: three launches (PREP, KIN, SPLITB); read per call
-    const bool k1 = k1env ? atoi(k1env) != 0 : true;
+    const bool k1 = s->opt_k1 != 0;                         // GPE_OPT_FUSED_K1 = 0: three launches (PREP, KIN, SPLITB)
     for (int64_t n = 0; n < nsteps; ++n) {
         // A holds the un-normalised state of the previous iteration; its scale sits in d_sums[NACC]
         int rc;
@@ -922,6 +958,24 @@ int gpe_sim_set_compact_weights(gpe_sim* s, double centre, const double* face_xy
     for (int k = 0; k < 8; ++k) s->w27[k] = v[k];
     s->custom27 = true;
     return GPE_OK;
+}
+
+int gpe_sim_set_option(gpe_sim* s, int option, int value) {
+    if (!s) return fail(GPE_ERR_INVALID_ARG, "null argument");
+    if (value != 0 && value != 1) return fail(GPE_ERR_INVALID_ARG, "option values are 0 or 1");
+    switch (option) {
+        case GPE_OPT_FUSED_K1: s->opt_k1 = value; return GPE_OK;
+        case GPE_OPT_RK4_GRAPH: s->opt_graph = value; return GPE_OK;
+        case GPE_OPT_PDL:
+            if (s->opt_pdl != value && s->rk4_exec) {   // the captured launches carry the old attribute
+                CU(cudaDeviceSynchronize());
+                cudaGraphExecDestroy(s->rk4_exec);
+                s->rk4_exec = nullptr;
+            }
+            s->opt_pdl = value;
+            return GPE_OK;
+        default: return fail(GPE_ERR_INVALID_ARG, "unknown option");
+    }
 }
 
 int gpe_sim_set_planes_per_block(gpe_sim* s, int kz) {

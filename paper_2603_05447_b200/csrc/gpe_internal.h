@@ -147,7 +147,8 @@ struct StageParams {
 
 // Launchers (gpe_kernels.cu).  dtype: GPE_C64 / GPE_C128; radius 1 or 2.  Return cudaError_t as int.
 // variant: 1 = 7-point, 2 = 13-point, 3 = 19-point higher-order compact (radius 1 + in-plane / z diagonals)
-int launch_stage(int dtype, int variant, int mode, const StageParams& p, void* stream);
+// pdl != 0: the launch carries the programmatic-stream-serialization attribute (the kernels call griddepcontrol)
+int launch_stage(int dtype, int variant, int mode, const StageParams& p, void* stream, int pdl);
 size_t stage_smem_bytes(int dtype, int variant);
 int stage_max_planes();   // upper bound of WorkRec::nz the stage kernels accept
 int launch_pack(int dtype, const void* canonical, void* storage, const int64_t* perm, int64_t n, void* stream);

@@ -6,6 +6,7 @@
 // Compiled with -ffp-contract=off: the mask must be bit-exact against an independent evaluation, so the
 // potential is evaluated in the fixed order of DESIGN.md R2 with one rounding per operation.
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstring>
 #include <limits>
@@ -191,14 +192,15 @@ int build_layout_from_potential(const gpe_box& box, const gpe_potential& pot, do
     for (int iz = 0; iz < box.nz; ++iz) { double z = coord(iz, box.nz, box.hz > 0.0 ? box.hz : box.h, box.center[2]); zz[iz] = pot.az * (z * z); }
 
     std::vector<std::vector<TileTmp>> rows(ntx);
-    bool oom = false;
+    std::atomic<bool> oom{false};   // set by any thread whose allocation fails (no exception may leave the region)
 #pragma omp parallel
     {
         std::vector<uint64_t> buf;
-        try { buf.resize((size_t)nty * box.nz); } catch (...) { oom = true; }
+        try { buf.resize((size_t)nty * box.nz); } catch (...) { oom.store(true, std::memory_order_relaxed); }
 #pragma omp for schedule(dynamic, 1)
         for (int i = 0; i < ntx; ++i) {
-            if (oom) continue;
+            if (oom.load(std::memory_order_relaxed)) continue;
+            try {
             std::fill(buf.begin(), buf.end(), 0ull);
             for (int lx = 0; lx < tx; ++lx) {
                 int ix = i * tx + lx;
@@ -225,9 +227,10 @@ int build_layout_from_potential(const gpe_box& box, const gpe_potential& pot, do
                 t.masks.assign(mrow + zlo, mrow + zhi);
                 rows[i].push_back(std::move(t));
             }
+            } catch (...) { oom.store(true, std::memory_order_relaxed); }
         }
     }
-    if (oom) { *err = "out of host memory in the layout builder"; return GPE_ERR_OUT_OF_MEMORY; }
+    if (oom.load()) { *err = "out of host memory in the layout builder"; return GPE_ERR_OUT_OF_MEMORY; }
     std::vector<TileTmp> tiles;
     for (int i = 0; i < ntx; ++i)
         for (auto& t : rows[i]) tiles.push_back(std::move(t));

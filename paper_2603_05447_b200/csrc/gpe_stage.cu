@@ -749,26 +749,32 @@ template <typename T, int R, int MODE, bool HOC, bool REAL> constexpr size_t sta
     return (size_t)(STAGE_WARPS * rows_per_lane<T>() / 2) * Geo<T, R, mode_has_aux(MODE), HOC, REAL>::STREAM_BYTES;
 }
 
+// where a stage launch goes: the stream, and whether it may start under programmatic dependent launch
+// (gpe_sim_set_option GPE_OPT_PDL; 0 = plain stream-ordered launches)
+struct LaunchAt {
+    cudaStream_t stream;
+    int pdl;
+};
+
 template <typename T, int R, int MODE, bool HOC, bool REAL>
-cudaError_t launch_one(const StageParams& p, cudaStream_t st) {
+cudaError_t launch_one(const StageParams& p, LaunchAt st) {
     constexpr int spb = STAGE_WARPS * rows_per_lane<T>() / 2;   // streams per block
     const int nblk = (p.n_work + spb - 1) / spb;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)nblk);
     cfg.blockDim = dim3(STAGE_THREADS);
     cfg.dynamicSmemBytes = stage_smem<T, R, MODE, HOC, REAL>();
-    cfg.stream = st;
+    cfg.stream = st.stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    static const int pdl = [] { const char* e = getenv("GPE_PDL"); return e ? atoi(e) : 1; }();   // GPE_PDL=0: plain launches
-    attr[0].val.programmaticStreamSerializationAllowed = pdl;
+    attr[0].val.programmaticStreamSerializationAllowed = st.pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, stage_kernel<T, R, MODE, rows_per_lane<T>(), HOC, REAL>, p);
 }
 
 template <typename T, int R, bool HOC>
-cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
+cudaError_t launch_mode(int mode, const StageParams& p, LaunchAt st) {
     switch (mode) {
         case MODE_APPLY: return launch_one<T, R, MODE_APPLY, HOC, false>(p, st);
         case MODE_S1: return launch_one<T, R, MODE_S1, HOC, false>(p, st);
@@ -788,7 +794,7 @@ cudaError_t launch_mode(int mode, const StageParams& p, cudaStream_t st) {
 
 // real-valued fp64 state: the operator and the imaginary-time modes only (real time needs the imaginary part)
 template <int R, bool HOC>
-cudaError_t launch_mode_real(int mode, const StageParams& p, cudaStream_t st) {
+cudaError_t launch_mode_real(int mode, const StageParams& p, LaunchAt st) {
     switch (mode) {
         case MODE_APPLY: return launch_one<double, R, MODE_APPLY, HOC, true>(p, st);
         case MODE_IMAG: return launch_one<double, R, MODE_IMAG, HOC, true>(p, st);
@@ -864,15 +870,15 @@ int kernels_configure() {
 }
 
 template <typename T>
-cudaError_t launch_variant(int variant, int mode, const StageParams& p, cudaStream_t st) {
+cudaError_t launch_variant(int variant, int mode, const StageParams& p, LaunchAt st) {
     if (variant == 1) return launch_mode<T, 1, false>(mode, p, st);
     if (variant == 2) return launch_mode<T, 2, false>(mode, p, st);
     if (variant == 3) return launch_mode<T, 1, true>(mode, p, st);
     return cudaErrorInvalidValue;
 }
 
-int launch_stage(int dtype, int variant, int mode, const StageParams& p, void* stream) {
-    cudaStream_t st = (cudaStream_t)stream;
+int launch_stage(int dtype, int variant, int mode, const StageParams& p, void* stream, int pdl) {
+    const LaunchAt st{(cudaStream_t)stream, pdl};
     if (p.n_work <= 0) return 0;
     if (dtype == GPE_R64) {
         if (variant == 1) return (int)launch_mode_real<1, false>(mode, p, st);

@@ -191,20 +191,25 @@ def test_imag_split_small_shell(P, stencil, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["complex128", "complex64", "float64"])
-@pytest.mark.parametrize("stencil", [7, 13, 19])
-def test_imag_split_k1_equals_three_launches(P, stencil, dtype, monkeypatch):
+@pytest.mark.parametrize("stencil", [7, 13, 19, 27])
+def test_imag_split_k1_equals_three_launches(P, stencil, dtype):
     """The paper's K1 (Eq. 7 half step and lazy scale applied to every value while it is staged, own
     and halo, then the first Euler half step) gives bit for bit what the separate pointwise launch followed by the
-    kinetic launch gives (GPE_K1=0): the same arithmetic at the same point, whichever tile stages the value."""
+    kinetic launch gives (gpe_sim_set_option GPE_OPT_FUSED_K1 = 0): the same arithmetic at the same point, whichever
+    tile stages the value.  Stencil 27 runs with caller-supplied weights and a non-zero corner weight, so the eight
+    corner reads of the diagonal tiles go through the folded load too."""
     w = I.small_shell(40, stencil, "complex128" if dtype == "float64" else dtype).with_(g=400.0)
-    box, pot, act = oracle_objs(w)
     grid = P.Grid.from_workload(w)
+    act = grid.active_indices()
     psi = I.make_psi0(w, act)
     psi = np.abs(psi).astype(np.float64) if dtype == "float64" else psi.astype(np.complex64 if dtype == "complex64" else np.complex128)
     out = []
-    for k1 in ("1", "0"):
-        monkeypatch.setenv("GPE_K1", k1)
+    for k1 in (1, 0):
         sim = P.Sim(grid, dtype, stencil, w.g)
+        sim.set_option(P.OPT_FUSED_K1, k1)
+        if stencil == 27:
+            h2 = w.h ** 2
+            sim.set_compact_weights(-64.0 / 15.0 / h2, [7.0 / 15.0 / h2] * 3, [0.1 / h2] * 3, 1.0 / 30.0 / h2)
         sim.set_psi_host(psi)
         n0 = sim.kernel_launches
         sim.run_imag_split(2e-3, 6)
@@ -219,7 +224,7 @@ def test_imag_split_k1_equals_three_launches(P, stencil, dtype, monkeypatch):
                                          ((6, 6, 6), 1.1, 6), ((19, 21, 37), 0.6, 8), ((1, 20, 33), 0.8, 9), ((24, 1, 1), 0.7, 10)])
 @pytest.mark.parametrize("stencil", [7, 13, 19])
 @pytest.mark.parametrize("kz", [32, 3, 1])
-def test_imag_split_k1_random_masks(P, dims, p, seed, stencil, kz, monkeypatch):
+def test_imag_split_k1_random_masks(P, dims, p, seed, stencil, kz):
     """K1 on random masks (holes everywhere, box faces touched, streams of 1-3 planes, boxes one point thick): the
     iteration against the oracle, and bit for bit against the three-launch form."""
     nx, ny, nz = dims
@@ -231,9 +236,9 @@ def test_imag_split_k1_random_masks(P, dims, p, seed, stencil, kz, monkeypatch):
     og = O.SparseGrid(box, act, RADIUS[stencil])
     psi = I.random_psi(seed + 100, act.size)
     out = []
-    for k1 in ("1", "0"):
-        monkeypatch.setenv("GPE_K1", k1)
+    for k1 in (1, 0):
         sim = P.Sim(grid, "complex128", stencil, w.g)
+        sim.set_option(P.OPT_FUSED_K1, k1)
         sim.set_planes_per_block(kz)
         sim.set_psi_host(psi)
         sim.run_imag_split(5e-3, 4)
@@ -522,6 +527,34 @@ def test_zero_state_has_no_renormalisation(P):
     assert rel_max(sim.get_psi_host(), O.run_imag(og, pot, w.g, 0.0, 1e-3, 2, psi, 13)) < 1e-12
 
 
+def test_replacing_the_state_discards_an_unreported_degenerate_flag(P):
+    """include/gpe.h, gpe_imag_step: the deferred GPE_ERR_STATE belongs to the state that raised it.  A zero state runs
+    through both imaginary-time forms with no reporting call in between; then the state is replaced (host copy, device
+    copy, re-gridding from another sim) and the next run, norm and read-back succeed and match the oracle."""
+    w = I.small_shell(24, 13)
+    box, pot, act, grid, sim = _make(P, w)
+    og = O.SparseGrid(box, act, 2)
+    zero = np.zeros(act.size, np.complex128)
+    psi = I.make_psi0(w, act)
+    ref = O.run_imag(og, pot, w.g, 0.0, 1e-3, 2, psi, 13)
+    src = P.Sim(grid, "complex128", 13, w.g)
+    src.set_psi_host(psi)
+    for replace in (lambda: sim.set_psi_host(psi), lambda: sim.set_psi(_dev(psi, "complex128")), lambda: sim.remap_from(src)):
+        sim.set_psi_host(zero)
+        sim.run_imag(1e-3, 3)
+        _torch().cuda.synchronize()                        # the flag is up and its copy has landed, nobody has asked yet
+        replace()
+        sim.run_imag(1e-3, 2)                              # would return GPE_ERR_STATE if the stale flag were still pending
+        assert abs(sim.norm() - 1.0) < 1e-12
+        assert rel_max(sim.get_psi_host(), ref) < 1e-12
+    # and a flag raised by the new state is still reported
+    sim.set_psi_host(zero)
+    sim.run_imag_split(1e-3, 2)
+    with pytest.raises(P.GpeError) as e:
+        sim.norm()
+    assert e.value.code == -5
+
+
 def test_staged_ramp_with_regridding(P):
     """The ramp as the paper runs it (PAPER.md:151-153): stage after stage of a linearly interpolated potential;
     at the end of each stage the grid post-selection is repeated with the threshold 5 max(mu_i, mu_i+1) and the
@@ -610,3 +643,71 @@ def test_graph_replay_is_bit_identical(P, dtype):
     sim.run_rk4(wr.dt, 20)
     og = O.SparseGrid(box, act, 2)
     assert rel_max(sim.get_psi_host(), O.run_rk4(og, pot, wr.g, 0.0, wr.dt, 20, psi.astype(np.complex128), 13)) < (1e-11 if dtype == "complex128" else 1e-4)
+
+
+
+@pytest.mark.parametrize("stencil", [13, 19])
+def test_graph_replay_dressed_static_at_nonzero_t0_and_after_knob_changes(P, stencil):
+    """gpe_run_rk4's graph path on the dressed potential: (a) Delta constant (delta0 == delta1) with the run starting
+    at t0 != 0; (b) a ramp that has already ended at t0 (Delta(t) = delta1 from there on); (c) re-entry after
+    gpe_sim_set_planes_per_block and, for the compact stencil, after gpe_sim_set_compact_weights -- each bit-identical
+    to the same run taken one step per call (runs of one step never use the graph)."""
+    def both_ways(sim, psi, t0, dt, n):
+        sim.set_psi_host(psi)
+        sim.time = t0
+        sim.run_rk4(dt, n)
+        got = sim.get_psi_host().copy()
+        assert abs(sim.time - (t0 + n * dt)) < 1e-15
+        sim.set_psi_host(psi)
+        for k in range(n):
+            sim.time = t0 + k * dt                          # step k of a run starts at t0 + k dt (a product, gpe.h)
+            sim.run_rk4(dt, 1)
+        assert np.array_equal(sim.get_psi_host(), got)
+        return got
+
+    w = I.small_shell(24, stencil)
+    box, pot, act, grid, sim = _make(P, w)
+    psi = I.make_psi0(w, act)
+    a = both_ways(sim, psi, 0.37, w.dt, 19)                 # 2 replays + 3 single steps
+    og = O.SparseGrid(box, act, 2)
+    assert rel_max(a, O.run_rk4(og, pot, w.g, 0.37, w.dt, 19, psi, stencil)) < 1e-11
+    sim.set_planes_per_block(5)                             # new work records: the graph is rebuilt, same numbers
+    assert np.array_equal(both_ways(sim, psi, 0.37, w.dt, 19), a)
+    if stencil == 19:
+        sim.set_compact_weights(-4.2 / w.h ** 2, [0.4 / w.h ** 2] * 3, [0.15 / w.h ** 2] * 3, 0.0)
+        b = both_ways(sim, psi, 0.37, w.dt, 16)
+        assert not np.array_equal(b, a)
+    # (b) the ramp 14 -> 22 ends at t = 0.05; from t0 = 0.06 on the potential is static at delta1
+    wr = w.with_(delta0=14.0, delta1=22.0, t_ramp=0.05)
+    box, pot, act, grid, sim = _make(P, wr)
+    psi = I.make_psi0(wr, act)
+    got = both_ways(sim, psi, 0.06, wr.dt, 17)
+    og = O.SparseGrid(box, act, 2)
+    assert rel_max(got, O.run_rk4(og, pot, wr.g, 0.06, wr.dt, 17, psi, stencil)) < 1e-11
+    # the same sim inside the ramp (no graph), then after it again (the kept graph is still the right one)
+    both_ways(sim, psi, 0.0, wr.dt, 17)
+    assert np.array_equal(both_ways(sim, psi, 0.06, wr.dt, 17), got)
+
+
+def test_sim_options_switch_between_bit_identical_forms(P):
+    """gpe_sim_set_option (include/gpe.h): the graph replay and programmatic dependent launch change how the launches
+    are issued, not what they compute; bad arguments are refused."""
+    w = I.config1()
+    box, pot, act, grid, sim = _make(P, w)
+    psi = I.make_psi0(w, act)
+    res = []
+    for graph, pdl in ((1, 1), (0, 1), (1, 0), (0, 0), (1, 1)):
+        sim.set_option(P.OPT_RK4_GRAPH, graph)
+        sim.set_option(P.OPT_PDL, pdl)
+        sim.set_psi_host(psi)
+        sim.time = 0.0
+        n0 = sim.kernel_launches
+        sim.run_rk4(w.dt, 24)
+        res.append(sim.get_psi_host().copy())
+        assert sim.kernel_launches - n0 == 24 * 4 + 2       # + pack and unpack: replayed launches are counted too
+    for r in res[1:]:
+        assert np.array_equal(r, res[0])
+    for opt, val in ((7, 1), (-1, 0), (P.OPT_PDL, 2), (P.OPT_FUSED_K1, -1)):
+        with pytest.raises(P.GpeError) as e:
+            sim.set_option(opt, val)
+        assert e.value.code == -1

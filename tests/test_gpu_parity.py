@@ -704,7 +704,7 @@ def test_sim_options_switch_between_bit_identical_forms(P):
         n0 = sim.kernel_launches
         sim.run_rk4(w.dt, 24)
         res.append(sim.get_psi_host().copy())
-        assert sim.kernel_launches - n0 == 24 * 4 + 2       # + pack and unpack: replayed launches are counted too
+        assert sim.kernel_launches - n0 == 24 * 4 + 1       # + the unpack of the read-back: replayed launches are counted too
     for r in res[1:]:
         assert np.array_equal(r, res[0])
     for opt, val in ((7, 1), (-1, 0), (P.OPT_PDL, 2), (P.OPT_FUSED_K1, -1)):
